@@ -1,0 +1,133 @@
+/*
+ * sw.h -- C ABI of libsw_b200: one Swendsen-Wang (SW) multi-cluster Monte Carlo step on one
+ * NVIDIA B200 (sm_100a), after arXiv 1403.7560 (Komura & Okabe), section 2.
+ *
+ * One SW step is
+ *   (1) active-bond generation between aligned nearest neighbours,
+ *   (2) cluster labelling = connected components of the active-bond graph,
+ *   (3) a new random value per cluster (Ising, Potts) or a reflection of the whole cluster with
+ *       probability 1/2 (XY, Wolff embedding) applied to every site,
+ * followed, on request, by the observables of PAPER.md:142-157 (Eq. 1-5).
+ * Lattices: periodic 2D square and 3D simple cubic.  Models: Ising (Eq. 1), q-state
+ * Potts (Eq. 2), classical XY with continuous fp32 angles (Eq. 3).  J = 1, beta = 1/T.
+ *
+ * Every step of the path runs in hand-written CUDA kernels; there is NO CPU fallback: without a
+ * usable CUDA device every call that needs one returns SW_ECUDA.
+ *
+ * Conventions (DESIGN.md section 3 lists every reading of the paper):
+ *   site index   i = x + L*y (+ L*L*z), x fastest; each site owns its +x, +y (, +z) bonds;
+ *   bond byte    bit k = the bond from site i to its +e_k neighbour is active;
+ *   label        minimum linear site index of the site's cluster (what label equivalence with
+ *                atomicMin from label = index converges to);
+ *   randoms      Philox4x32-10, key = (seed low, seed high), counter = (site, t low, t high,
+ *                domain); domain 0: word k decides bond k of the site, word 3 is the new value of
+ *                the cluster rooted at the site; domain 2: start configuration; domain 3: XY
+ *                direction of step t.  t = 0-based index of the step being executed.
+ *
+ * Pointers: `sw_ctx *` is an opaque HOST pointer owned by the library.  All `host_*` arguments
+ * are HOST pointers owned by the caller.  `device_workspace` (sw_create_in) is a DEVICE pointer
+ * owned by the caller, which must outlive the context.  Nothing else crosses the boundary.
+ *
+ * Errors: every call returns an int status (SW_OK = 0, negative on error), never throws and never
+ * aborts.  sw_last_error() returns a thread-local description of the last failure.  CUDA errors
+ * are sticky in the context: after one, every later call on that context returns SW_ECUDA.
+ *
+ * Threading: one context = one CUDA stream; calls on one context are not re-entrant.
+ */
+#ifndef SW_B200_H
+#define SW_B200_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sw_ctx sw_ctx;
+
+enum { SW_ISING = 0, SW_POTTS = 1, SW_XY = 2 };
+enum { SW_OK = 0, SW_EINVAL = -1, SW_ENOMEM = -2, SW_ECUDA = -3, SW_ESTATE = -4 };
+
+/* ---- the four calls of the hot path ------------------------------------------------------- */
+
+/* Create a context for a dim-dimensional (2 or 3) periodic lattice of linear size L with a seeded
+ * random start configuration (device_function_spinset) and step counter t = 0.
+ *   L      multiple of 32 ("nx ... multiple of 32"), L >= 32, L^dim <= 2^31;
+ *   model  SW_ISING | SW_POTTS | SW_XY;  q: number of Potts states, 2..255 (ignored otherwise);
+ *   beta   J/T with J = 1, finite, >= 0;  seed: Philox key.
+ * Device memory comes from cudaMalloc and the context owns a new non-blocking stream.
+ * On failure *out = NULL. */
+int sw_create(sw_ctx **out, int dim, int L, int model, int q, double beta, uint64_t seed);
+
+/* Same, but the context lives in caller-provided DEVICE memory (e.g. a torch tensor from the
+ * caching allocator) of at least sw_workspace_bytes() bytes, 256-byte aligned, and launches on
+ * the caller's CUDA stream (`cuda_stream` is a cudaStream_t passed as void *; NULL = the legacy
+ * default stream).  The caller keeps ownership of both. */
+int sw_create_in(sw_ctx **out, int dim, int L, int model, int q, double beta, uint64_t seed,
+                 void *device_workspace, size_t workspace_bytes, void *cuda_stream);
+/* Bytes sw_create_in needs; 0 if the arguments are invalid. */
+size_t sw_workspace_bytes(int dim, int L, int model, int q);
+
+/* n >= 0 SW steps, asynchronous on the context's stream (no host sync). */
+int sw_step(sw_ctx *c, int n);
+
+/* Instantaneous, extensive observables of the CURRENT configuration.
+ * Synchronises the stream.  Any output pointer may be NULL.
+ *   Ising: E = -sum_<ij> s_i s_j (Eq. 1), M = sum_i s_i (Eq. 4, signed), M2 = M^2, M4 = M^4.
+ *   Potts: E = number of unequal nearest-neighbour pairs (Eq. 2), M2 = (q sum_k n_k^2 - N^2)/(q-1)
+ *          (Eq. 5), M = sqrt(M2), M4 = M2^2.
+ *   XY:    E = -sum_<ij> cos(theta_i - theta_j) (Eq. 3), M = |sum_i (cos, sin)|, M2, M4 likewise.
+ * Averages, the specific heat and the moment ratio (Eq. 6) are the caller's job. */
+int sw_observables(sw_ctx *c, double *host_E, double *host_M, double *host_M2, double *host_M4);
+
+/* Destroy the context (synchronises its stream first).  NULL is a no-op. */
+int sw_destroy(sw_ctx *c);
+
+const char *sw_last_error(void);
+
+/* ---- state accessors (parity tests, checkpoint/restore, end-to-end host buffers) ---------- */
+
+/* Number of sites N = L^dim and index t of the next step. */
+size_t sw_num_sites(const sw_ctx *c);
+uint64_t sw_step_index(const sw_ctx *c);
+
+/* Copy the configuration to / from a HOST buffer of exactly N elements: int8 (Ising, +-1),
+ * uint8 (Potts, 0..q-1) or float32 (XY angle in [0, 2 pi]).  sw_set_spins also sets the step
+ * counter (state = (spins, seed, t), because the generator is counter-based).  Both synchronise.
+ * Values outside the model's range are not checked. */
+int sw_get_spins(sw_ctx *c, void *host_dst, size_t bytes);
+int sw_set_spins(sw_ctx *c, const void *host_src, size_t bytes, uint64_t step);
+
+/* Bond bytes (N) and flattened labels (N x uint32) of the LAST executed step; SW_ESTATE if no
+ * step ran since create / sw_set_spins. */
+int sw_get_bonds(sw_ctx *c, uint8_t *host_dst, size_t bytes);
+int sw_get_labels(sw_ctx *c, uint32_t *host_dst, size_t bytes);
+
+/* Exact integer sums of the current configuration.  Ising: *host_E = -sum s_i s_j,
+ * host_M_or_nk[0] = sum s_i (n >= 1).  Potts: *host_E = #unequal pairs, host_M_or_nk[k] = n_k for
+ * k < min(n, q).  SW_EINVAL for XY. */
+int sw_get_counts(sw_ctx *c, int64_t *host_E, int64_t *host_M_or_nk, int n);
+
+/* XY: direction r = (rx, ry) and reflection constant c = (2 phi + pi) mod 2 pi of the LAST step. */
+int sw_get_xy_dir(sw_ctx *c, float *host_rx, float *host_ry, float *host_c);
+/* XY test hook: use the angle phi for every following step instead of the Philox draw. */
+int sw_force_xy_phi(sw_ctx *c, int enable, double phi);
+
+/* Labelling counters of the LAST step (north_star: "labelling-iteration counts"); filled only
+ * when the context was switched to counting mode with sw_set_counting(c, 1), which makes the
+ * kernels slower.  out[0] = tile-border bonds examined, out[1] = active ones (unions attempted),
+ * out[2] = unions that linked two roots, out[3] = union retries, out[4] = total find hops in the
+ * merge, out[5] = max find hops of one call in the merge, out[6] = total root-chase hops in the
+ * flip kernel, out[7] = max hops of one chase. */
+int sw_set_counting(sw_ctx *c, int enable);
+int sw_get_label_stats(sw_ctx *c, uint64_t *host_out, int n);
+
+/* Philox4x32-10 exactly as the kernels compute it, evaluated on the device for `count` (counter,
+ * key) pairs: host_ctr = count x 4 words, host_key = count x 2 words, host_out = count x 4 words.
+ * Lets the tests pin the GPU generator to the known-answer vectors. */
+int sw_philox_selftest(const uint32_t *host_ctr, const uint32_t *host_key, uint32_t *host_out, int count);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,528 @@
+// sw_api.cu -- host driver and C ABI (include/sw.h) of libsw_b200.
+// Launch sequencing of one Swendsen-Wang step: k_bond_label -> k_merge -> k_flip,
+// all asynchronous on the context's stream; no host synchronisation inside sw_step.
+#include "../../include/sw.h"
+#include "sw_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+
+using namespace swk;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string &msg)
+{
+    g_err = msg;
+    return code;
+}
+
+// One tile configuration = the three tiled kernels instantiated for it.
+struct TileOps {
+    int tx, ty, tz, nt;
+    size_t smem_bond_label, smem_flip;
+    void (*bond_label)(const Params);
+    void (*merge)(const Params);
+    void (*flip)(const Params);
+};
+
+template <int DIM, int MODEL, int TX, int TY, int TZ>
+TileOps make_ops()
+{
+    using G = TileGeom<DIM, MODEL, TX, TY, TZ>;
+    constexpr int NS = G::NS;
+    constexpr int NT = NS / 8 > 1024 ? 1024 : (NS / 8 < 128 ? 128 : NS / 8);
+    TileOps o;
+    o.tx = TX; o.ty = TY; o.tz = TZ; o.nt = NT;
+    o.smem_bond_label = G::SMEM_BOND_LABEL;
+    o.smem_flip = G::SMEM_FLIP;
+    o.bond_label = k_bond_label<DIM, MODEL, TX, TY, TZ, NT>;
+    o.merge = k_merge<DIM, TX, TY, TZ>;
+    o.flip = k_flip<DIM, MODEL, TX, TY, TZ, NT>;
+    return o;
+}
+
+// Tile menu.  TX is a multiple of 32 (rows are warps); TY, TZ are powers of two <= 32, so they divide
+// every admissible L (multiple of 32); TX > 32 needs L % TX == 0.
+template <int MODEL>
+bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
+{
+#define SW_TILE2(X, Y) if (dim == 2 && tx == X && ty == Y) { o = make_ops<2, MODEL, X, Y, 1>(); return true; }
+#define SW_TILE3(X, Y, Z) if (dim == 3 && tx == X && ty == Y && tz == Z) { o = make_ops<3, MODEL, X, Y, Z>(); return true; }
+    SW_TILE2(32, 32)
+    SW_TILE2(64, 32)
+    SW_TILE2(128, 16)
+    SW_TILE2(128, 32)
+    SW_TILE3(32, 8, 8)
+    SW_TILE3(32, 16, 8)
+    SW_TILE3(32, 16, 16)
+    SW_TILE3(64, 8, 8)
+#undef SW_TILE2
+#undef SW_TILE3
+    return false;
+}
+
+bool pick_ops_model(int model, int dim, int tx, int ty, int tz, TileOps &o)
+{
+    if (model == SW_ISING) return pick_ops<ISING>(dim, tx, ty, tz, o);
+    if (model == SW_POTTS) return pick_ops<POTTS>(dim, tx, ty, tz, o);
+    return pick_ops<XY>(dim, tx, ty, tz, o);
+}
+
+size_t align256(size_t v) { return (v + 255) / 256 * 256; }
+
+bool valid_args(int dim, int L, int model, int q, double beta, bool check_beta)
+{
+    if (dim != 2 && dim != 3) return false;
+    if (L < 32 || L % 32 != 0) return false;
+    if (model != SW_ISING && model != SW_POTTS && model != SW_XY) return false;
+    if (model == SW_POTTS && (q < 2 || q > 255)) return false;
+    if (check_beta && !(std::isfinite(beta) && beta >= 0.0)) return false;
+    double n = std::pow((double)L, dim);
+    if (n > 2147483648.0) return false;
+    return true;
+}
+
+struct Layout { size_t spins, bonds, labels, acc, total; };
+
+Layout layout(int dim, int L, int model)
+{
+    size_t N = 1;
+    for (int a = 0; a < dim; ++a) N *= (size_t)L;
+    Layout l;
+    size_t off = 0;
+    l.spins = off; off += align256(N * (model == SW_XY ? 4 : 1));
+    l.bonds = off; off += align256(N);
+    l.labels = off; off += align256(N * 4);
+    l.acc = off; off += align256(sizeof(Acc));
+    l.total = off;
+    return l;
+}
+
+}  // namespace
+
+struct sw_ctx {
+    int dim, L, model, q;
+    double beta;
+    uint64_t seed, t;
+    size_t N;
+    Params p;
+    TileOps ops;
+    cudaStream_t stream;
+    void *workspace;
+    bool own_workspace, own_stream;
+    bool stepped;      // bonds/labels of a step are available
+    bool labels_flat;
+    bool M_fresh;      // acc holds the magnetisation sums of the current configuration
+    bool E_fresh;
+    int force_phi;
+    double forced_phi;
+    float rx, ry, crefl;
+    int sticky;
+};
+
+namespace {
+
+int cuda_fail(sw_ctx *c, cudaError_t e, const char *what)
+{
+    if (c) c->sticky = 1;
+    return fail(SW_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define SW_CUDA(c, call)                                         \
+    do {                                                         \
+        cudaError_t e_ = (call);                                 \
+        if (e_ != cudaSuccess) return cuda_fail(c, e_, #call);   \
+    } while (0)
+
+int check_ctx(sw_ctx *c)
+{
+    if (!c) return fail(SW_EINVAL, "null context");
+    if (c->sticky) return fail(SW_ECUDA, "context is in a sticky CUDA error state");
+    return SW_OK;
+}
+
+dim3 tile_grid(const sw_ctx *c)
+{
+    return dim3(c->L / c->ops.tx, c->L / c->ops.ty, c->dim == 3 ? c->L / c->ops.tz : 1);
+}
+
+uint32_t threshold32(double prob)
+{
+    double v = std::floor(prob * 4294967296.0);
+    if (v >= 4294967295.0) return 4294967295u;
+    if (v <= 0.0) return 0u;
+    return (uint32_t)v;
+}
+
+template <int MODEL>
+void launch_init(sw_ctx *c)
+{
+    k_init<MODEL><<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->p);
+}
+
+template <int DIM, int MODEL>
+void launch_measure_dm(sw_ctx *c, bool with_m)
+{
+    const unsigned g = (unsigned)(c->N / 256);
+    if (with_m) k_measure<DIM, MODEL, true><<<g, 256, 0, c->stream>>>(c->p);
+    else k_measure<DIM, MODEL, false><<<g, 256, 0, c->stream>>>(c->p);
+}
+
+void launch_measure(sw_ctx *c, bool with_m)
+{
+    if (c->dim == 2) {
+        if (c->model == SW_ISING) launch_measure_dm<2, ISING>(c, with_m);
+        else if (c->model == SW_POTTS) launch_measure_dm<2, POTTS>(c, with_m);
+        else launch_measure_dm<2, XY>(c, with_m);
+    } else {
+        if (c->model == SW_ISING) launch_measure_dm<3, ISING>(c, with_m);
+        else if (c->model == SW_POTTS) launch_measure_dm<3, POTTS>(c, with_m);
+        else launch_measure_dm<3, XY>(c, with_m);
+    }
+}
+
+// Make acc hold E (and M) of the current configuration.
+int refresh_observables(sw_ctx *c)
+{
+    if (c->E_fresh && c->M_fresh) return SW_OK;
+    const bool with_m = !c->M_fresh;
+    // E_int and E_xy are the first 16 bytes of Acc; the magnetisation sums follow.
+    const size_t clear = with_m ? offsetof(Acc, stats) : offsetof(Acc, M_int);
+    SW_CUDA(c, cudaMemsetAsync(c->p.acc, 0, clear, c->stream));
+    launch_measure(c, with_m);
+    SW_CUDA(c, cudaGetLastError());
+    c->E_fresh = c->M_fresh = true;
+    return SW_OK;
+}
+
+int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, uint64_t seed,
+                  void *workspace, size_t workspace_bytes, void *stream, bool external)
+{
+    if (!out) return fail(SW_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!valid_args(dim, L, model, q, beta, true))
+        return fail(SW_EINVAL, "invalid arguments (dim 2|3, L multiple of 32 with L^dim <= 2^31, model, 2<=q<=255, beta>=0)");
+    const Layout lay = layout(dim, L, model);
+    if (external) {
+        if (!workspace || workspace_bytes < lay.total || ((uintptr_t)workspace & 255u))
+            return fail(SW_EINVAL, "device workspace missing, too small or not 256-byte aligned");
+    }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(SW_ECUDA, "no usable CUDA device (this library has no CPU fallback)");
+    }
+    sw_ctx *c = new (std::nothrow) sw_ctx();
+    if (!c) return fail(SW_ENOMEM, "host allocation failed");
+    c->dim = dim; c->L = L; c->model = model; c->q = (model == SW_POTTS) ? q : 0;
+    c->beta = beta; c->seed = seed; c->t = 0;
+    c->N = lay.total ? 1 : 0;
+    for (int a = 0; a < dim; ++a) c->N *= (size_t)L;
+    c->own_workspace = !external; c->own_stream = !external;
+    c->stream = external ? (cudaStream_t)stream : nullptr;
+    c->workspace = workspace;
+    if (!external) {
+        e = cudaMalloc(&c->workspace, lay.total);
+        if (e != cudaSuccess) { cudaGetLastError(); delete c; return fail(SW_ENOMEM, "cudaMalloc failed"); }
+        e = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) { cudaFree(c->workspace); delete c; return fail(SW_ECUDA, "cudaStreamCreate failed"); }
+    }
+    // tile choice: default per dimension, SW_B200_TILE=TXxTYxTZ overrides (tuning knob)
+    int tx = 32, ty = (dim == 2) ? 32 : 8, tz = (dim == 2) ? 1 : 8;
+    if (dim == 2 && L % 128 == 0) { tx = 128; ty = 32; }
+    if (const char *env = std::getenv("SW_B200_TILE")) {
+        int ex = 0, ey = 0, ez = 1;
+        if (std::sscanf(env, "%dx%dx%d", &ex, &ey, &ez) >= 2) { tx = ex; ty = ey; tz = (dim == 2) ? 1 : ez; }
+    }
+    bool ok = (L % tx == 0) && (L % ty == 0) && (L % tz == 0) && pick_ops_model(model, dim, tx, ty, tz, c->ops);
+    if (!ok) {
+        tx = 32; ty = (dim == 2) ? 32 : 8; tz = (dim == 2) ? 1 : 8;
+        pick_ops_model(model, dim, tx, ty, tz, c->ops);
+    }
+    char *base = (char *)c->workspace;
+    Params &p = c->p;
+    p.spins = base + lay.spins;
+    p.bonds = (uint8_t *)(base + lay.bonds);
+    p.labels = (uint32_t *)(base + lay.labels);
+    p.acc = (Acc *)(base + lay.acc);
+    p.L = (uint32_t)L; p.N = (uint32_t)c->N;
+    p.log2L = -1;
+    for (int s = 0; s < 31; ++s) if ((1u << s) == (uint32_t)L) p.log2L = s;
+    p.k0 = (uint32_t)(seed & 0xffffffffu); p.k1 = (uint32_t)(seed >> 32);
+    p.t_lo = p.t_hi = 0;
+    // PAPER.md:96 (garbled "p = 1 e^{2J/T}"): Ising p = 1 - exp(-2 beta); PAPER.md:152 + Eq. 2: Potts
+    // p = 1 - exp(-beta).  The decision is the integer compare word < floor(p 2^32).
+    const double prob = (model == SW_ISING) ? -std::expm1(-2.0 * beta) : -std::expm1(-beta);
+    p.P32 = threshold32(prob);
+    p.q = c->q;
+    p.rx = 1.f; p.ry = 0.f; p.crefl = 0.f; p.m2beta = (float)(-2.0 * beta);
+    p.counting = 0;
+    c->force_phi = 0; c->forced_phi = 0.0; c->rx = c->ry = c->crefl = 0.f; c->sticky = 0;
+
+    auto bail = [&](cudaError_t err, const char *what) {
+        std::string m = std::string(what) + ": " + cudaGetErrorString(err);
+        if (c->own_workspace) cudaFree(c->workspace);
+        if (c->own_stream) cudaStreamDestroy(c->stream);
+        delete c;
+        return fail(SW_ECUDA, m);
+    };
+    e = cudaFuncSetAttribute(c->ops.bond_label, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ops.smem_bond_label);
+    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_bond_label)");
+    e = cudaFuncSetAttribute(c->ops.flip, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ops.smem_flip);
+    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_flip)");
+    e = cudaMemsetAsync(p.acc, 0, sizeof(Acc), c->stream);
+    if (e != cudaSuccess) return bail(e, "cudaMemsetAsync");
+    if (model == SW_ISING) launch_init<ISING>(c);
+    else if (model == SW_POTTS) launch_init<POTTS>(c);
+    else launch_init<XY>(c);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return bail(e, "k_init launch");
+    c->stepped = false; c->labels_flat = false; c->M_fresh = false; c->E_fresh = false;
+    *out = c;
+    return SW_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *sw_last_error(void) { return g_err.c_str(); }
+
+size_t sw_workspace_bytes(int dim, int L, int model, int q)
+{
+    if (!valid_args(dim, L, model, q, 0.0, false)) return 0;
+    return layout(dim, L, model).total;
+}
+
+int sw_create(sw_ctx **out, int dim, int L, int model, int q, double beta, uint64_t seed)
+{
+    return create_common(out, dim, L, model, q, beta, seed, nullptr, 0, nullptr, false);
+}
+
+int sw_create_in(sw_ctx **out, int dim, int L, int model, int q, double beta, uint64_t seed,
+                 void *device_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    return create_common(out, dim, L, model, q, beta, seed, device_workspace, workspace_bytes, cuda_stream, true);
+}
+
+int sw_step(sw_ctx *c, int n)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (n < 0) return fail(SW_EINVAL, "n < 0");
+    const dim3 grid = tile_grid(c);
+    const uint32_t slots = (uint32_t)(c->N / c->ops.tx + c->N / c->ops.ty + (c->dim == 3 ? c->N / c->ops.tz : 0));
+    for (int s = 0; s < n; ++s) {
+        Params &p = c->p;
+        p.t_lo = (uint32_t)(c->t & 0xffffffffu);
+        p.t_hi = (uint32_t)(c->t >> 32);
+        if (c->model == SW_XY) {
+            // PAPER.md:159 "randomly chosen" direction: phi uniform from one Philox word (domain 3),
+            // r = (cos phi, sin phi) rounded to fp32; reflection constant c = (2 phi + pi) mod 2 pi.
+            const double two_pi = 6.283185307179586476925286766559;
+            const uint4 w = philox4x32_10(0u, p.t_lo, p.t_hi, DOM_XYDIR, p.k0, p.k1);
+            double phi = (double)w.x * (two_pi / 4294967296.0);
+            if (c->force_phi) phi = c->forced_phi;
+            p.rx = c->rx = (float)std::cos(phi);
+            p.ry = c->ry = (float)std::sin(phi);
+            p.crefl = c->crefl = (float)std::fmod(2.0 * phi + two_pi / 2.0, two_pi);
+        }
+        if (p.counting) SW_CUDA(c, cudaMemsetAsync(p.acc->stats, 0, sizeof(p.acc->stats), c->stream));
+        c->ops.bond_label<<<grid, c->ops.nt, c->ops.smem_bond_label, c->stream>>>(p);
+        c->ops.merge<<<(slots + 255) / 256, 256, 0, c->stream>>>(p);
+        c->ops.flip<<<grid, c->ops.nt, c->ops.smem_flip, c->stream>>>(p);
+        c->t += 1;
+    }
+    if (n > 0) {
+        SW_CUDA(c, cudaGetLastError());
+        c->stepped = true; c->labels_flat = false; c->M_fresh = true; c->E_fresh = false;
+    }
+    return SW_OK;
+}
+
+int sw_observables(sw_ctx *c, double *E, double *M, double *M2, double *M4)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    rc = refresh_observables(c);
+    if (rc) return rc;
+    Acc h;
+    SW_CUDA(c, cudaMemcpyAsync(&h, c->p.acc, offsetof(Acc, stats), cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    double e, m, m2;
+    if (c->model == SW_ISING) {
+        e = (double)(long long)h.E_int;
+        m = (double)(long long)h.M_int;
+        m2 = m * m;
+    } else if (c->model == SW_POTTS) {
+        // Eq. (5): M^2 = (q sum_k n_k^2 - N^2) / (q - 1)
+        double s2 = 0.0;
+        for (int k = 0; k < c->q; ++k) s2 += (double)h.nk[k] * (double)h.nk[k];
+        const double Nd = (double)c->N;
+        e = (double)(long long)h.E_int;
+        m2 = ((double)c->q * s2 - Nd * Nd) / (double)(c->q - 1);
+        m = std::sqrt(m2);
+    } else {
+        e = h.E_xy;
+        m2 = h.mx * h.mx + h.my * h.my;
+        m = std::sqrt(m2);
+    }
+    if (E) *E = e;
+    if (M) *M = m;
+    if (M2) *M2 = m2;
+    if (M4) *M4 = m2 * m2;
+    return SW_OK;
+}
+
+int sw_destroy(sw_ctx *c)
+{
+    if (!c) return SW_OK;
+    cudaStreamSynchronize(c->stream);
+    if (c->own_workspace) cudaFree(c->workspace);
+    if (c->own_stream) cudaStreamDestroy(c->stream);
+    cudaGetLastError();
+    delete c;
+    return SW_OK;
+}
+
+size_t sw_num_sites(const sw_ctx *c) { return c ? c->N : 0; }
+uint64_t sw_step_index(const sw_ctx *c) { return c ? c->t : 0; }
+
+int sw_get_spins(sw_ctx *c, void *dst, size_t bytes)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    const size_t want = c->N * (c->model == SW_XY ? 4 : 1);
+    if (!dst || bytes != want) return fail(SW_EINVAL, "sw_get_spins: buffer must hold exactly N elements");
+    SW_CUDA(c, cudaMemcpyAsync(dst, c->p.spins, want, cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SW_OK;
+}
+
+int sw_set_spins(sw_ctx *c, const void *src, size_t bytes, uint64_t step)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    const size_t want = c->N * (c->model == SW_XY ? 4 : 1);
+    if (!src || bytes != want) return fail(SW_EINVAL, "sw_set_spins: buffer must hold exactly N elements");
+    SW_CUDA(c, cudaMemcpyAsync(c->p.spins, src, want, cudaMemcpyHostToDevice, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->t = step;
+    c->stepped = false; c->labels_flat = false; c->M_fresh = false; c->E_fresh = false;
+    return SW_OK;
+}
+
+int sw_get_bonds(sw_ctx *c, uint8_t *dst, size_t bytes)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (!c->stepped) return fail(SW_ESTATE, "no step since create / sw_set_spins");
+    if (!dst || bytes != c->N) return fail(SW_EINVAL, "sw_get_bonds: buffer must hold exactly N bytes");
+    SW_CUDA(c, cudaMemcpyAsync(dst, c->p.bonds, c->N, cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SW_OK;
+}
+
+int sw_get_labels(sw_ctx *c, uint32_t *dst, size_t bytes)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (!c->stepped) return fail(SW_ESTATE, "no step since create / sw_set_spins");
+    if (!dst || bytes != c->N * 4) return fail(SW_EINVAL, "sw_get_labels: buffer must hold exactly N uint32");
+    if (!c->labels_flat) {
+        k_flatten<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->p);
+        SW_CUDA(c, cudaGetLastError());
+        c->labels_flat = true;
+    }
+    SW_CUDA(c, cudaMemcpyAsync(dst, c->p.labels, c->N * 4, cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SW_OK;
+}
+
+int sw_get_counts(sw_ctx *c, int64_t *E, int64_t *M_or_nk, int n)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (c->model == SW_XY) return fail(SW_EINVAL, "sw_get_counts: integer sums are not defined for XY");
+    rc = refresh_observables(c);
+    if (rc) return rc;
+    Acc h;
+    SW_CUDA(c, cudaMemcpyAsync(&h, c->p.acc, offsetof(Acc, stats), cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (E) *E = (int64_t)h.E_int;
+    if (M_or_nk) {
+        if (c->model == SW_ISING) { if (n >= 1) M_or_nk[0] = (int64_t)h.M_int; }
+        else for (int k = 0; k < n && k < c->q; ++k) M_or_nk[k] = (int64_t)h.nk[k];
+    }
+    return SW_OK;
+}
+
+int sw_get_xy_dir(sw_ctx *c, float *rx, float *ry, float *cr)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (c->model != SW_XY) return fail(SW_EINVAL, "not an XY context");
+    if (!c->stepped) return fail(SW_ESTATE, "no step since create / sw_set_spins");
+    if (rx) *rx = c->rx;
+    if (ry) *ry = c->ry;
+    if (cr) *cr = c->crefl;
+    return SW_OK;
+}
+
+int sw_force_xy_phi(sw_ctx *c, int enable, double phi)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (c->model != SW_XY) return fail(SW_EINVAL, "not an XY context");
+    c->force_phi = enable; c->forced_phi = phi;
+    return SW_OK;
+}
+
+int sw_set_counting(sw_ctx *c, int enable)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    c->p.counting = enable ? 1 : 0;
+    return SW_OK;
+}
+
+int sw_get_label_stats(sw_ctx *c, uint64_t *out, int n)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (!out || n < 0) return fail(SW_EINVAL, "sw_get_label_stats: bad buffer");
+    unsigned long long h[8];
+    SW_CUDA(c, cudaMemcpyAsync(h, c->p.acc->stats, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < n && k < 8; ++k) out[k] = h[k];
+    return SW_OK;
+}
+
+int sw_philox_selftest(const uint32_t *ctr, const uint32_t *key, uint32_t *out, int count)
+{
+    if (!ctr || !key || !out || count <= 0) return fail(SW_EINVAL, "sw_philox_selftest: bad arguments");
+    uint32_t *d = nullptr;
+    const size_t n = (size_t)count;
+    SW_CUDA(nullptr, cudaMalloc(&d, n * 10 * sizeof(uint32_t)));
+    uint32_t *dc = d, *dk = d + 4 * n, *dout = d + 6 * n;
+    cudaError_t e = cudaMemcpy(dc, ctr, n * 16, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(dk, key, n * 8, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_philox_selftest<<<(count + 127) / 128, 128>>>(dc, dk, dout, count);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(out, dout, n * 16, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "sw_philox_selftest");
+    return SW_OK;
+}
+
+}  // extern "C"

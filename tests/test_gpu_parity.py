@@ -1,0 +1,206 @@
+"""GPU-vs-oracle parity through the C ABI (all -m gpu).
+
+Ising / Potts: bonds, labels, spins and the integer E / M / n_k must be IDENTICAL after every step
+(BASELINE.json north_star).  The oracle (oracle/, sequential C, BFS) shares no code with the CUDA
+path; both start from the same seeded inputs (paper_1403_7560_b200.inputs) or their own Philox INIT.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from lattice_ref import components_min_label, plus_neighbours
+
+pytestmark = pytest.mark.gpu
+
+TC2 = 2.269185
+T3 = 4.5115
+TP3 = 1.0 / math.log(1.0 + math.sqrt(3.0))
+
+
+def _mods():
+    from oracle import sw_oracle as orc
+    import paper_1403_7560_b200 as sw
+    return sw, orc
+
+
+def _compare_step(g, o, tag):
+    """After one step on both sides: everything must be bit-identical."""
+    bg, bo = g.bonds(), o.bonds()
+    assert np.array_equal(bg, bo), f"{tag}: bonds differ at {np.flatnonzero(bg != bo)[:8]}"
+    lg, lo = g.labels(), o.labels()
+    assert np.array_equal(lg, lo), f"{tag}: labels differ at {np.flatnonzero(lg != lo)[:8]}"
+    sg, so = g.spins(), o.spins()
+    assert np.array_equal(sg, so), f"{tag}: spins differ at {np.flatnonzero(sg != so)[:8]}"
+    assert g.counts() == o.counts(), f"{tag}: integer E / M differ"
+
+
+def test_philox_device_known_answers():
+    """The device generator against the Random123 known-answer vectors (tests/golden)."""
+    import os
+    sw, _ = _mods()
+    from stats import golden_rows
+    rows = golden_rows(os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt"))
+    ctr = [[int(x, 16) for x in r[0:4]] for r in rows]
+    key = [[int(x, 16) for x in r[4:6]] for r in rows]
+    want = [[int(x, 16) for x in r[6:10]] for r in rows]
+    got = sw.philox_selftest(ctr, key)
+    assert got.tolist() == want
+
+
+@pytest.mark.parametrize("dim,L,model,q,T,steps", [
+    (2, 64, 0, 0, TC2, 1000),      # config C1, the whole 1000-step trajectory
+    (2, 32, 0, 0, TC2, 200),       # one tile: every wrap bond goes through the merge kernel
+    (2, 96, 0, 0, TC2, 60),        # L not a power of two, 3 x 3 tiles of 32
+    (2, 256, 0, 0, TC2, 60),
+    (2, 512, 0, 0, TC2, 20),
+    (2, 256, 1, 3, TP3, 60),
+    (2, 128, 1, 7, 0.8, 30),
+    (3, 32, 0, 0, T3, 60),
+    (3, 64, 0, 0, T3, 30),
+    (3, 96, 0, 0, T3, 6),
+    (3, 64, 1, 3, 1.8, 20),        # 3D Potts (one of the paper's six programs)
+    (3, 32, 1, 20, 1.2, 20),       # q > 8: shared-memory histogram path
+])
+def test_full_trajectory_bit_exact(dim, L, model, q, T, steps):
+    sw, orc = _mods()
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=1)
+    o = orc.Oracle(dim, L, model, q, 1.0 / T, 1)
+    assert np.array_equal(g.spins(), o.spins()), "seeded start differs"
+    assert g.counts() == o.counts()
+    for t in range(steps):
+        g.step(1)
+        o.step(1)
+        _compare_step(g, o, f"dim{dim} L{L} model{model} t={t}")
+    assert g.t == o.t == steps
+    e, m, m2, m4 = g.observables()
+    assert (e, m, m2, m4) == pytest.approx(o.observables(), rel=1e-14)
+
+
+@pytest.mark.parametrize("tile", ["32x32", "64x32", "128x16", "128x32"])
+def test_tile_menu_2d(tile, monkeypatch):
+    sw, orc = _mods()
+    monkeypatch.setenv("SW_B200_TILE", tile)
+    g = sw.SwendsenWang(2, 256, 0, 0, 1.0 / TC2, seed=5)
+    o = orc.Oracle(2, 256, 0, 0, 1.0 / TC2, 5)
+    for t in range(25):
+        g.step(1)
+        o.step(1)
+        _compare_step(g, o, f"tile {tile} t={t}")
+
+
+@pytest.mark.parametrize("tile", ["32x8x8", "32x16x8", "32x16x16", "64x8x8"])
+def test_tile_menu_3d(tile, monkeypatch):
+    sw, orc = _mods()
+    monkeypatch.setenv("SW_B200_TILE", tile)
+    g = sw.SwendsenWang(3, 64, 0, 0, 1.0 / T3, seed=5)
+    o = orc.Oracle(3, 64, 0, 0, 1.0 / T3, 5)
+    for t in range(12):
+        g.step(1)
+        o.step(1)
+        _compare_step(g, o, f"tile {tile} t={t}")
+
+
+@pytest.mark.parametrize("dim,L,model,q", [(2, 128, 0, 0), (3, 32, 0, 0), (2, 128, 1, 3)])
+def test_edge_beta_zero_and_cold_start(dim, L, model, q):
+    """I5: beta = 0 -> no bonds, label[i] = i; large beta + aligned start -> one cluster, label 0."""
+    sw, orc = _mods()
+    from paper_1403_7560_b200 import inputs
+    N = L ** dim
+    g = sw.SwendsenWang(dim, L, model, q, 0.0, seed=3)
+    o = orc.Oracle(dim, L, model, q, 0.0, 3)
+    g.step(1)
+    o.step(1)
+    assert not g.bonds().any()
+    assert np.array_equal(g.labels(), np.arange(N, dtype=np.uint32))
+    _compare_step(g, o, "beta=0")
+    g = sw.SwendsenWang(dim, L, model, q, 40.0, seed=3)
+    o = orc.Oracle(dim, L, model, q, 40.0, 3)
+    cold = inputs.aligned_spins(model, N)
+    g.set_spins(cold, 7)
+    o.set_spins(cold, 7)
+    g.step(1)
+    o.step(1)
+    assert (g.bonds() == (1 << dim) - 1).all()
+    assert not g.labels().any()
+    assert len(np.unique(g.spins())) == 1
+    _compare_step(g, o, "cold")
+
+
+@pytest.mark.parametrize("dim,L,model,q,T", [(2, 256, 0, 0, 1.5), (3, 64, 0, 0, 3.0), (2, 256, 1, 4, 0.7)])
+def test_injected_structured_states(dim, L, model, q, T):
+    """Stripes and block domains at low T: long clusters crossing many tiles and the wrap faces."""
+    sw, orc = _mods()
+    from paper_1403_7560_b200 import inputs
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=11)
+    o = orc.Oracle(dim, L, model, q, 1.0 / T, 11)
+    states = [inputs.striped_spins(model, dim, L, 5, max(q, 2)),
+              inputs.domain_spins(model, dim, L, 24, max(q, 2), seed=2),
+              inputs.random_spins(model, L ** dim, q, seed=4)]
+    for k, s in enumerate(states):
+        g.set_spins(s, 1000 * k)
+        o.set_spins(s, 1000 * k)
+        for t in range(3):
+            g.step(1)
+            o.step(1)
+            _compare_step(g, o, f"state {k} t={t}")
+
+
+def test_labels_are_components_independent_check():
+    """I2/I3 with scipy's connected_components (neither the oracle's BFS nor the GPU's union-find)."""
+    sw, _ = _mods()
+    g = sw.SwendsenWang(3, 64, 0, 0, 1.0 / T3, seed=2)
+    g.step(30)
+    before = g.spins()
+    g.step(1)
+    bonds, labels, after = g.bonds(), g.labels(), g.spins()
+    ref, ncomp = components_min_label(3, 64, bonds)
+    assert np.array_equal(labels.astype(np.int64), ref)
+    nb = plus_neighbours(3, 64)
+    for k in range(3):
+        on = (bonds >> k) & 1 == 1
+        assert (before[on] == before[nb[k]][on]).all()      # I1: bonds join only aligned spins
+        assert (after[on] == after[nb[k]][on]).all()        # I4: clusters are uniform after the flip
+    assert len(np.unique(labels)) == ncomp
+
+
+def test_determinism_and_step_batching():
+    """I6: same (seed, spins, t) -> same result; sw_step(n) == n x sw_step(1); library-owned memory path."""
+    sw, _ = _mods()
+    a = sw.SwendsenWang(2, 256, 0, 0, 1.0 / TC2, seed=9)
+    b = sw.SwendsenWang(2, 256, 0, 0, 1.0 / TC2, seed=9, use_torch=False)
+    a.step(40)
+    for _ in range(40):
+        b.step(1)
+    assert np.array_equal(a.spins(), b.spins())
+    assert np.array_equal(a.labels(), b.labels())
+    assert a.counts() == b.counts()
+    c = sw.SwendsenWang(2, 256, 0, 0, 1.0 / TC2, seed=10)
+    c.step(5)
+    assert not np.array_equal(a.spins(), c.spins())
+
+
+def test_ising_equals_potts_q2():
+    """R1: Ising(beta) == Potts(q=2, 2 beta) bit for bit under s = 2k - 1."""
+    sw, _ = _mods()
+    beta = 1.0 / TC2
+    a = sw.SwendsenWang(2, 128, 0, 0, beta, seed=4)
+    b = sw.SwendsenWang(2, 128, 1, 2, 2.0 * beta, seed=4)
+    for t in range(20):
+        a.step(1)
+        b.step(1)
+        assert np.array_equal(a.spins(), 2 * b.spins().astype(np.int8) - 1)
+        assert np.array_equal(a.labels(), b.labels())
+        assert np.array_equal(a.bonds(), b.bonds())
+
+
+def test_state_errors():
+    sw, _ = _mods()
+    g = sw.SwendsenWang(2, 64, 0, 0, 0.4, seed=1)
+    with pytest.raises(sw.SwError) as ei:
+        g.bonds()
+    assert ei.value.code == -4
+    with pytest.raises(sw.SwError):
+        g.set_spins(np.zeros(10, dtype=np.int8), 0)
+    g.step(0)
+    assert g.t == 0
