@@ -122,6 +122,14 @@ int sw_force_xy_phi(sw_ctx *c, int enable, double phi);
 int sw_set_counting(sw_ctx *c, int enable);
 int sw_get_label_stats(sw_ctx *c, uint64_t *host_out, int n);
 
+/* Per-kernel device times.  With timing enabled, sw_step brackets each of the three kernels of a
+ * step (k_bond_label, k_merge, k_flip) with CUDA events on the context's stream and synchronises
+ * after every step (a measurement mode, slower than the asynchronous default).
+ * sw_get_kernel_times returns the accumulated milliseconds per kernel (host_ms[0..2]) and the number
+ * of steps accumulated (*host_steps) since timing was enabled, then clears the accumulators. */
+int sw_set_kernel_timing(sw_ctx *c, int enable);
+int sw_get_kernel_times(sw_ctx *c, double *host_ms, int n, uint64_t *host_steps);
+
 /* Philox4x32-10 exactly as the kernels compute it, evaluated on the device for `count` (counter,
  * key) pairs: host_ctr = count x 4 words, host_key = count x 2 words, host_out = count x 4 words.
  * Lets the tests pin the GPU generator to the known-answer vectors. */

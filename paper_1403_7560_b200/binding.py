@@ -54,6 +54,8 @@ def lib():
     L.sw_force_xy_phi.argtypes = [vp, i32, dbl]
     L.sw_set_counting.argtypes = [vp, i32]
     L.sw_get_label_stats.argtypes = [vp, C.POINTER(u64), i32]
+    L.sw_set_kernel_timing.argtypes = [vp, i32]
+    L.sw_get_kernel_times.argtypes = [vp, C.POINTER(dbl), i32, C.POINTER(u64)]
     L.sw_philox_selftest.argtypes = [vp, vp, vp, i32]
     _lib = L
     return _lib
@@ -178,3 +180,13 @@ class SwendsenWang:
         names = ("border_bonds", "active_border_bonds", "unions_linked", "union_retries",
                  "merge_find_hops", "merge_find_hops_max", "chase_hops", "chase_hops_max")
         return dict(zip(names, [int(x) for x in out]))
+
+    def set_kernel_timing(self, enable):
+        _check(lib().sw_set_kernel_timing(self._h, int(bool(enable))))
+
+    def kernel_times(self):
+        """(ms per kernel [k_bond_label, k_merge, k_flip], steps) accumulated in timing mode."""
+        ms = (C.c_double * 3)()
+        n = C.c_uint64()
+        _check(lib().sw_get_kernel_times(self._h, ms, 3, C.byref(n)))
+        return [float(x) for x in ms], int(n.value)

@@ -125,6 +125,10 @@ struct sw_ctx {
     double forced_phi;
     float rx, ry, crefl;
     int sticky;
+    int timing;            // per-kernel event timing mode
+    cudaEvent_t ev[4];
+    double kernel_ms[3];
+    uint64_t timed_steps;
 };
 
 namespace {
@@ -266,6 +270,9 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     p.rx = 1.f; p.ry = 0.f; p.crefl = 0.f; p.m2beta = (float)(-2.0 * beta);
     p.counting = 0;
     c->force_phi = 0; c->forced_phi = 0.0; c->rx = c->ry = c->crefl = 0.f; c->sticky = 0;
+    c->timing = 0; c->timed_steps = 0;
+    for (int k = 0; k < 3; ++k) c->kernel_ms[k] = 0.0;
+    for (int k = 0; k < 4; ++k) c->ev[k] = nullptr;
 
     auto bail = [&](cudaError_t err, const char *what) {
         std::string m = std::string(what) + ": " + cudaGetErrorString(err);
@@ -336,9 +343,22 @@ int sw_step(sw_ctx *c, int n)
             p.crefl = c->crefl = (float)std::fmod(2.0 * phi + two_pi / 2.0, two_pi);
         }
         if (p.counting) SW_CUDA(c, cudaMemsetAsync(p.acc->stats, 0, sizeof(p.acc->stats), c->stream));
+        if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[0], c->stream));
         c->ops.bond_label<<<grid, c->ops.nt, c->ops.smem_bond_label, c->stream>>>(p);
+        if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[1], c->stream));
         c->ops.merge<<<(slots + 255) / 256, 256, 0, c->stream>>>(p);
+        if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[2], c->stream));
         c->ops.flip<<<grid, c->ops.nt, c->ops.smem_flip, c->stream>>>(p);
+        if (c->timing) {
+            SW_CUDA(c, cudaEventRecord(c->ev[3], c->stream));
+            SW_CUDA(c, cudaEventSynchronize(c->ev[3]));
+            for (int k = 0; k < 3; ++k) {
+                float ms = 0.f;
+                SW_CUDA(c, cudaEventElapsedTime(&ms, c->ev[k], c->ev[k + 1]));
+                c->kernel_ms[k] += (double)ms;
+            }
+            c->timed_steps += 1;
+        }
         c->t += 1;
     }
     if (n > 0) {
@@ -386,6 +406,7 @@ int sw_destroy(sw_ctx *c)
 {
     if (!c) return SW_OK;
     cudaStreamSynchronize(c->stream);
+    for (int k = 0; k < 4; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     if (c->own_workspace) cudaFree(c->workspace);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     cudaGetLastError();
@@ -503,6 +524,32 @@ int sw_get_label_stats(sw_ctx *c, uint64_t *out, int n)
     SW_CUDA(c, cudaMemcpyAsync(h, c->p.acc->stats, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
     for (int k = 0; k < n && k < 8; ++k) out[k] = h[k];
+    return SW_OK;
+}
+
+int sw_set_kernel_timing(sw_ctx *c, int enable)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (enable) {
+        for (int k = 0; k < 4; ++k)
+            if (!c->ev[k]) SW_CUDA(c, cudaEventCreate(&c->ev[k]));
+    }
+    c->timing = enable ? 1 : 0;
+    c->timed_steps = 0;
+    for (int k = 0; k < 3; ++k) c->kernel_ms[k] = 0.0;
+    return SW_OK;
+}
+
+int sw_get_kernel_times(sw_ctx *c, double *ms, int n, uint64_t *steps)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (!ms || n < 0) return fail(SW_EINVAL, "sw_get_kernel_times: bad buffer");
+    for (int k = 0; k < n && k < 3; ++k) ms[k] = c->kernel_ms[k];
+    if (steps) *steps = c->timed_steps;
+    c->timed_steps = 0;
+    for (int k = 0; k < 3; ++k) c->kernel_ms[k] = 0.0;
     return SW_OK;
 }
 
