@@ -241,7 +241,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     }
     // tile choice: default per dimension, SW_B200_TILE=TXxTYxTZ overrides (tuning knob)
     int tx = 32, ty = (dim == 2) ? 32 : 8, tz = (dim == 2) ? 1 : 8;
-    if (dim == 2 && L % 128 == 0) { tx = 128; ty = 32; }
+    if (dim == 2 && L % 128 == 0) { tx = 128; ty = 16; }
     if (const char *env = std::getenv("SW_B200_TILE")) {
         int ex = 0, ey = 0, ez = 1;
         if (std::sscanf(env, "%dx%dx%d", &ex, &ey, &ez) >= 2) { tx = ex; ty = ey; tz = (dim == 2) ? 1 : ez; }

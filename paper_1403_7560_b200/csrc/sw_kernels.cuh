@@ -140,11 +140,12 @@ __global__ void __launch_bounds__(256) k_init(const Params p)
 
 // ------------------------------------------------------------------------------------------------
 // k_bond_label: one CTA per TX x TY x TZ tile.
-//   stage   spins (XY: projections a_i = r . s_i) of the tile and its +x/+y/+z faces -> smem
+//   (XY only) stage the projections a_i = r . s_i of the tile and its +x/+y/+z faces in smem
 //   rows    one warp per row of 32 sites along x: Philox(site, t) -> bond bits; the ballot of the
-//           x-bond bits gives every lane the start of its run, so x-connectivity costs no union
-//   unions  y/z bonds (and x bonds across 32-lane segments) -> atomicMin union-find in smem
-//   flatten label[i] = global index of the tile-local root; bond byte written for the merge kernel
+//           x-bond bits gives every lane the start of its run, so x-connectivity costs no union;
+//           active y/z bonds inside the tile are compacted into a work list (ballot + popc)
+//   unions  the work list is processed densely, one bond per thread: atomicMin union-find in smem
+//   flatten label[i] = global index of the tile-local root
 // Local index order (lx fastest, then ly, lz) is monotone in the global index inside a tile, so the
 // tile-local minimum is the global minimum over the tile's part of the cluster.
 // ------------------------------------------------------------------------------------------------
@@ -152,11 +153,14 @@ template <int DIM, int MODEL, int TX, int TY, int TZ>
 struct TileGeom {
     static constexpr int SX = TX + 1, SY = TY + 1, SZ = (DIM == 3) ? TZ + 1 : 1;
     static constexpr int NS = TX * TY * TZ;
-    static constexpr int NSTAGE = SX * SY * SZ;
-    using val_t = typename ValT<MODEL>::type;
-    static constexpr size_t VAL_BYTES = ((size_t)NSTAGE * sizeof(val_t) + 15) / 16 * 16;
-    static constexpr size_t SMEM_BOND_LABEL = VAL_BYTES + (size_t)NS * 4 + (size_t)NS;
-    static constexpr size_t SMEM_FLIP = (size_t)NS * 4 + (size_t)NS;
+    static_assert(NS <= 8192, "work-list entries keep the local index in 13 bits");
+    static constexpr int NSTAGE = (MODEL == XY) ? SX * SY * SZ : 0;
+    static constexpr int NWORK = 2 * NS + NS / 32;  // every y/z bond of the tile + the x seams
+    static constexpr size_t VAL_BYTES = ((size_t)NSTAGE * 4 + 15) / 16 * 16;
+    static constexpr size_t OFF_LAB = VAL_BYTES;
+    static constexpr size_t OFF_WORK = OFF_LAB + (size_t)NS * 4;
+    static constexpr size_t SMEM_BOND_LABEL = OFF_WORK + (size_t)NWORK * 2;
+    static constexpr size_t SMEM_FLIP = (size_t)NS * 4 + (size_t)NS + (size_t)NS * 2;
 };
 
 template <int DIM, int MODEL, int TX, int TY, int TZ, int NT>
@@ -164,79 +168,109 @@ __global__ void __launch_bounds__(NT) k_bond_label(const Params p)
 {
     static_assert(TX % 32 == 0, "rows are warps");
     using G = TileGeom<DIM, MODEL, TX, TY, TZ>;
-    using val_t = typename G::val_t;
-    constexpr int SX = G::SX, SY = G::SY, NS = G::NS;
+    constexpr int SX = G::SX, SY = G::SY, SZ = G::SZ, NS = G::NS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    val_t *val_s = reinterpret_cast<val_t *>(smem_raw);
-    uint32_t *lab_s = reinterpret_cast<uint32_t *>(smem_raw + G::VAL_BYTES);
-    uint8_t *bond_s = reinterpret_cast<uint8_t *>(smem_raw + G::VAL_BYTES + (size_t)NS * 4);
+    float *val_s = reinterpret_cast<float *>(smem_raw);
+    uint32_t *lab_s = reinterpret_cast<uint32_t *>(smem_raw + G::OFF_LAB);
+    uint16_t *work_s = reinterpret_cast<uint16_t *>(smem_raw + G::OFF_WORK);
+    __shared__ int count_s;
 
     const uint32_t L = p.L;
     const uint32_t x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = (DIM == 3) ? blockIdx.z * TZ : 0u;
     const int tid = threadIdx.x;
-
-    for (int s = tid; s < G::NSTAGE; s += NT) {
-        const int lx = s % SX, ly = (s / SX) % SY, lz = s / (SX * SY);
-        const int nh = (lx == TX) + (ly == TY) + ((DIM == 3 && lz == TZ) ? 1 : 0);
-        if (nh >= 2) continue;  // edges and corners of the halo are never read
-        uint32_t gx = x0 + lx, gy = y0 + ly, gz = z0 + lz;
-        if (gx == L) gx = 0;
-        if (gy == L) gy = 0;
-        if (DIM == 3 && gz == L) gz = 0;
-        const uint32_t g = gx + L * (gy + L * gz);
-        if (MODEL == XY) {
-            float sn, cs;
-            sincosf(((const float *)p.spins)[g], &sn, &cs);
-            val_s[s] = (val_t)(p.rx * cs + p.ry * sn);  // a_i = r . s_i
-        } else {
-            val_s[s] = (val_t)((const uint8_t *)p.spins)[g];
-        }
-    }
-    __syncthreads();
-
     constexpr int ROWS = NS / 32, NW = NT / 32;
     const int lane = tid & 31, warp = tid >> 5;
 
-    for (int row = warp; row < ROWS; row += NW) {
-        const int li = row * 32 + lane;
-        const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
-        const int si = (lz * SY + ly) * SX + lx;
-        const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
-        const uint4 w = philox4x32_10(g, p.t_lo, p.t_hi, DOM_SITE, p.k0, p.k1);
-        const val_t v = val_s[si];
-        uint32_t b = 0;
-        if (MODEL == XY) {
-            // Wolff embedding (PAPER.md:88, 159): aligned iff a_i a_j > 0, p = 1 - exp(-2 beta a_i a_j)
-            const float scale = 5.9604644775390625e-8f;  // 2^-24
-            const float px = (float)v * (float)val_s[si + 1];
-            const float py = (float)v * (float)val_s[si + SX];
-            if (px > 0.f && (float)(w.x >> 8) * scale < -expm1f(p.m2beta * px)) b |= 1u;
-            if (py > 0.f && (float)(w.y >> 8) * scale < -expm1f(p.m2beta * py)) b |= 2u;
-            if (DIM == 3) {
-                const float pz = (float)v * (float)val_s[si + SX * SY];
-                if (pz > 0.f && (float)(w.z >> 8) * scale < -expm1f(p.m2beta * pz)) b |= 4u;
+    if (tid == 0) count_s = 0;
+    if (MODEL == XY) {
+        // a_i = r . s_i for the tile and its three plus-faces, one staged row per warp
+        for (int r = warp; r < SY * SZ; r += NW) {
+            const int ly = r % SY, lz = r / SY;
+            const bool face = (ly == TY) || (DIM == 3 && lz == TZ);
+            if (ly == TY && DIM == 3 && lz == TZ) continue;
+            uint32_t gy = y0 + ly, gz = z0 + lz;
+            if (gy == L) gy = 0;
+            if (DIM == 3 && gz == L) gz = 0;
+            const uint32_t rowbase = L * (gy + L * gz);
+            for (int lx = lane; lx < SX; lx += 32) {
+                if (face && lx == TX) continue;
+                uint32_t gx = x0 + lx;
+                if (gx == L) gx = 0;
+                float sn, cs;
+                sincosf(((const float *)p.spins)[rowbase + gx], &sn, &cs);
+                val_s[(lz * SY + ly) * SX + lx] = p.rx * cs + p.ry * sn;
             }
-        } else {
-            // a bond between equal neighbours is active with probability p
-            if (v == val_s[si + 1] && w.x < p.P32) b |= 1u;
-            if (v == val_s[si + SX] && w.y < p.P32) b |= 2u;
-            if (DIM == 3 && v == val_s[si + SX * SY] && w.z < p.P32) b |= 4u;
         }
-        const uint32_t xm = __ballot_sync(FULL, b & 1u);
-        const uint32_t zeros = ~xm & ((1u << lane) - 1u);  // lanes below me whose +x bond is off
-        const int start = zeros ? 32 - __clz(zeros) : 0;
-        lab_s[li] = (uint32_t)(row * 32 + start);
-        bond_s[li] = (uint8_t)b;
     }
     __syncthreads();
 
     for (int row = warp; row < ROWS; row += NW) {
         const int li = row * 32 + lane;
         const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
-        const uint32_t b = bond_s[li];
-        if ((b & 2u) && ly < TY - 1) union_s(lab_s, li, li + TX);
-        if (DIM == 3 && (b & 4u) && lz < TZ - 1) union_s(lab_s, li, li + TX * TY);
-        if (TX > 32 && (b & 1u) && lane == 31 && lx < TX - 1) union_s(lab_s, li, li + 1);
+        const uint32_t gx = x0 + lx, gy = y0 + ly, gz = z0 + lz;
+        const uint32_t g = gx + L * (gy + L * gz);
+        const uint4 w = philox4x32_10(g, p.t_lo, p.t_hi, DOM_SITE, p.k0, p.k1);
+        uint32_t b = 0;
+        if (MODEL == XY) {
+            // Wolff embedding (PAPER.md:88, 159): aligned iff a_i a_j > 0, p = 1 - exp(-2 beta a_i a_j)
+            const int si = (lz * SY + ly) * SX + lx;
+            const float scale = 5.9604644775390625e-8f;  // 2^-24
+            const float v = val_s[si];
+            const float px = v * val_s[si + 1];
+            const float py = v * val_s[si + SX];
+            if (px > 0.f && (float)(w.x >> 8) * scale < -expm1f(p.m2beta * px)) b |= 1u;
+            if (py > 0.f && (float)(w.y >> 8) * scale < -expm1f(p.m2beta * py)) b |= 2u;
+            if (DIM == 3) {
+                const float pz = v * val_s[si + SX * SY];
+                if (pz > 0.f && (float)(w.z >> 8) * scale < -expm1f(p.m2beta * pz)) b |= 4u;
+            }
+        } else {
+            // a bond between equal neighbours is active with probability p.
+            // Spins straight from global memory (the +y/+z rows hit L1: other warps load them as theirs).
+            const uint8_t *sp = (const uint8_t *)p.spins;
+            const uint32_t v = sp[g];
+            uint32_t vx = __shfl_down_sync(FULL, v, 1);
+            if (lane == 31) vx = sp[(gx + 1 == L) ? g - (L - 1) : g + 1];
+            const uint32_t vy = sp[(gy + 1 == L) ? g - L * (L - 1) : g + L];
+            if (v == vx && w.x < p.P32) b |= 1u;
+            if (v == vy && w.y < p.P32) b |= 2u;
+            if (DIM == 3) {
+                const uint32_t LL = L * L;
+                const uint32_t vz = sp[(gz + 1 == L) ? g - LL * (L - 1) : g + LL];
+                if (v == vz && w.z < p.P32) b |= 4u;
+            }
+        }
+        p.bonds[g] = (uint8_t)b;
+        const uint32_t xm = __ballot_sync(FULL, b & 1u);
+        const uint32_t below = (1u << lane) - 1u;
+        const uint32_t zeros = ~xm & below;  // lanes below me whose +x bond is off
+        const int start = zeros ? 32 - __clz(zeros) : 0;
+        lab_s[li] = (uint32_t)(row * 32 + start);
+        // compact the bonds that need a union: +y / +z inside the tile, +x across a 32-lane seam
+        const bool wy = (b & 2u) && ly < TY - 1;
+        const bool wz = DIM == 3 && (b & 4u) && lz < TZ - 1;
+        const bool wx = TX > 32 && (b & 1u) && lane == 31 && lx < TX - 1;
+        const uint32_t my = __ballot_sync(FULL, wy), mz = __ballot_sync(FULL, wz);
+        const int nx = (TX > 32) ? (int)((__ballot_sync(FULL, wx) >> 31) & 1u) : 0;
+        const int ny = __popc(my), nz = __popc(mz);
+        int base = 0;
+        if (lane == 0 && ny + nz + nx > 0) base = atomicAdd(&count_s, ny + nz + nx);
+        base = __shfl_sync(FULL, base, 0);
+        if (wy) work_s[base + __popc(my & below)] = (uint16_t)(li | (1u << 13));
+        if (wz) work_s[base + ny + __popc(mz & below)] = (uint16_t)(li | (2u << 13));
+        if (wx) work_s[base + ny + nz] = (uint16_t)li;
+    }
+    __syncthreads();
+
+    const int nwork = count_s;
+    for (int e0 = 0; e0 < nwork; e0 += NT) {
+        const int e = e0 + tid;
+        if (e < nwork) {
+            const uint32_t wk = work_s[e];
+            const uint32_t a = wk & 0x1fffu, d = wk >> 13;
+            union_s(lab_s, a, a + (d == 0 ? 1u : (d == 1 ? (uint32_t)TX : (uint32_t)(TX * TY))));
+        }
+        __syncwarp();
     }
     __syncthreads();
 
@@ -245,9 +279,9 @@ __global__ void __launch_bounds__(NT) k_bond_label(const Params p)
         const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
         const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
         const uint32_t r = find_s(lab_s, li);
+        __syncwarp();
         const int rx = r % TX, ry = (r / TX) % TY, rz = r / (TX * TY);
         p.labels[g] = (x0 + rx) + L * ((y0 + ry) + L * (z0 + rz));
-        p.bonds[g] = bond_s[li];
     }
 }
 
@@ -326,11 +360,13 @@ __global__ void __launch_bounds__(256) k_merge(const Params p)
 
 // ------------------------------------------------------------------------------------------------
 // k_flip: one CTA per tile.
-//   phase A  sites whose parent is themselves or lies outside the tile (the former tile-local
-//            roots) chase the global root r, draw the cluster's new value from word 3 of
-//            Philox(r, t) and park (r, draw) in smem; the others park a tile-local pointer
-//   phase B  the others follow the tile-local pointers in smem to a parked entry
-//   then     new spin / XY reflection written in place, magnetisation sums reduced per CTA
+//   phase A   every site reads its parent; sites whose parent is themselves or lies outside the tile
+//             (the former tile-local roots) are compacted into a list, the others park a tile-local
+//             pointer in smem
+//   phase A2  the list is processed densely, one root per thread: chase the global root r, draw the
+//             cluster's new value from word 3 of Philox(r, t), park (r, draw) in smem
+//   phase B   the other sites follow the tile-local pointers in smem to a parked entry
+//   then      new spin / XY reflection written in place, magnetisation sums reduced per CTA
 // ------------------------------------------------------------------------------------------------
 constexpr uint32_t LOCAL_PTR = 0x80000000u;
 
@@ -341,21 +377,25 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
     constexpr int NS = G::NS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint32_t *res_s = reinterpret_cast<uint32_t *>(smem_raw);
-    uint8_t *draw_s = reinterpret_cast<uint8_t *>(smem_raw + (size_t)NS * 4);
+    uint16_t *root_s = reinterpret_cast<uint16_t *>(smem_raw + (size_t)NS * 4);
+    uint8_t *draw_s = reinterpret_cast<uint8_t *>(smem_raw + (size_t)NS * 6);
     __shared__ unsigned long long hist_s[256];
     __shared__ double red_s[2][32];
+    __shared__ int count_s;
 
     const uint32_t L = p.L;
     const uint32_t x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = (DIM == 3) ? blockIdx.z * TZ : 0u;
     const int tid = threadIdx.x;
     constexpr int ROWS = NS / 32, NW = NT / 32;
     const int lane = tid & 31, warp = tid >> 5;
+    const uint32_t below = (1u << lane) - 1u;
 
+    if (tid == 0) count_s = 0;
     if (MODEL == POTTS) {
         for (int k = tid; k < 256; k += NT) hist_s[k] = 0ull;
     }
+    __syncthreads();
 
-    unsigned chase_hops = 0, chase_max = 0;
     for (int row = warp; row < ROWS; row += NW) {
         const int li = row * 32 + lane;
         const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
@@ -365,8 +405,23 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
         decode(p, par, px, py, pz);
         const uint32_t dx = px - x0, dy = py - y0, dz = pz - z0;
         const bool in_tile = dx < (uint32_t)TX && dy < (uint32_t)TY && dz < (uint32_t)TZ;
-        if (par == g || !in_tile) {
-            uint32_t r = par, n;
+        const bool is_root = (par == g) || !in_tile;
+        res_s[li] = is_root ? par : (LOCAL_PTR | (dx + TX * (dy + TY * dz)));
+        const uint32_t m = __ballot_sync(FULL, is_root);
+        int base = 0;
+        if (lane == 0 && m) base = atomicAdd(&count_s, __popc(m));
+        base = __shfl_sync(FULL, base, 0);
+        if (is_root) root_s[base + __popc(m & below)] = (uint16_t)li;
+    }
+    __syncthreads();
+
+    const int nroots = count_s;
+    unsigned chase_hops = 0, chase_max = 0;
+    for (int e0 = 0; e0 < nroots; e0 += NT) {
+        const int e = e0 + tid;
+        if (e < nroots) {
+            const int li = root_s[e];
+            uint32_t r = res_s[li], n;
             unsigned h = 0;
             while ((n = p.labels[r]) != r) { r = n; ++h; }
             chase_hops += h;
@@ -375,9 +430,8 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
             res_s[li] = r;
             draw_s[li] = (MODEL == POTTS) ? (uint8_t)(((unsigned long long)w * (unsigned)p.q) >> 32)
                                           : (uint8_t)(w >> 31);
-        } else {
-            res_s[li] = LOCAL_PTR | (dx + TX * (dy + TY * dz));
         }
+        __syncwarp();
     }
     __syncthreads();
 
@@ -389,6 +443,7 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
         const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
         uint32_t at = li, v = res_s[li];
         while (v & LOCAL_PTR) { at = v & ~LOCAL_PTR; v = res_s[at]; }
+        __syncwarp();
         const uint32_t d = draw_s[at];
         if (MODEL == ISING) {
             // "All spins in each cluster are set randomly to +1 or -1"
