@@ -53,7 +53,8 @@ enum { SW_OK = 0, SW_EINVAL = -1, SW_ENOMEM = -2, SW_ECUDA = -3, SW_ESTATE = -4 
 /* Create a context for a dim-dimensional (2 or 3) periodic lattice of linear size L with a seeded
  * random start configuration (device_function_spinset) and step counter t = 0.
  *   L      multiple of 32 ("nx ... multiple of 32"), L >= 32, L^dim <= 2^31;
- *   model  SW_ISING | SW_POTTS | SW_XY;  q: number of Potts states, 2..255 (ignored otherwise);
+ *   model  SW_ISING | SW_POTTS | SW_XY;  q: number of Potts states, 2..255 (ignored otherwise),
+ *          with L^dim * 2^ceil(log2 q) <= 2^32 (a label word holds a site address and a state);
  *   beta   J/T with J = 1, finite, >= 0;  seed: Philox key.
  * Device memory comes from cudaMalloc and the context owns a new non-blocking stream.
  * On failure *out = NULL. */
@@ -98,8 +99,15 @@ uint64_t sw_step_index(const sw_ctx *c);
 int sw_get_spins(sw_ctx *c, void *host_dst, size_t bytes);
 int sw_set_spins(sw_ctx *c, const void *host_src, size_t bytes, uint64_t step);
 
-/* Bond bytes (N) and flattened labels (N x uint32) of the LAST executed step; SW_ESTATE if no
- * step ran since create / sw_set_spins. */
+/* Bond bytes (N) and cluster labels (N x uint32, label = minimum linear site index of the cluster)
+ * of the LAST executed step; SW_ESTATE if no step ran since create / sw_set_spins.
+ * The step itself keeps bonds on chip and labels as packed parent pointers in a tiled order, so
+ *   - bond bytes exist only if recording was switched on BEFORE the step with
+ *     sw_set_record_bonds(c, 1) (default off; the same kernels then also store one byte per site);
+ *     otherwise sw_get_bonds returns SW_ESTATE;
+ *   - sw_get_labels converts on request (an extra kernel and N x 4 bytes of scratch device memory
+ *     that live only for the call; SW_ENOMEM if that allocation fails). */
+int sw_set_record_bonds(sw_ctx *c, int enable);
 int sw_get_bonds(sw_ctx *c, uint8_t *host_dst, size_t bytes);
 int sw_get_labels(sw_ctx *c, uint32_t *host_dst, size_t bytes);
 
@@ -115,10 +123,10 @@ int sw_force_xy_phi(sw_ctx *c, int enable, double phi);
 
 /* Labelling counters of the LAST step (north_star: "labelling-iteration counts"); filled only
  * when the context was switched to counting mode with sw_set_counting(c, 1), which makes the
- * kernels slower.  out[0] = tile-border bonds examined, out[1] = active ones (unions attempted),
- * out[2] = unions that linked two roots, out[3] = union retries, out[4] = total find hops in the
- * merge, out[5] = max find hops of one call in the merge, out[6] = total root-chase hops in the
- * flip kernel, out[7] = max hops of one chase. */
+ * kernels slower.  out[0] = tile-face bond slots examined, out[1] = active ones (unions attempted),
+ * out[2] = unions that linked two roots, out[3] = union retries (lost atomicCAS), out[4] = total
+ * find hops in the merge, out[5] = max find hops of one union, out[6] = total root-chase hops in
+ * the flip kernel, out[7] = max chase hops of one thread (16 sites). */
 int sw_set_counting(sw_ctx *c, int enable);
 int sw_get_label_stats(sw_ctx *c, uint64_t *host_out, int n);
 

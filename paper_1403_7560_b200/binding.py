@@ -47,6 +47,7 @@ def lib():
     L.sw_step_index.restype = u64
     L.sw_get_spins.argtypes = [vp, vp, sz]
     L.sw_set_spins.argtypes = [vp, vp, sz, u64]
+    L.sw_set_record_bonds.argtypes = [vp, i32]
     L.sw_get_bonds.argtypes = [vp, vp, sz]
     L.sw_get_labels.argtypes = [vp, vp, sz]
     L.sw_get_counts.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), i32]
@@ -81,7 +82,7 @@ class SwendsenWang:
     use_torch=True (default) places the context in a torch CUDA tensor and on torch's current stream
     (sw_create_in); use_torch=False lets the library cudaMalloc and own a stream (sw_create)."""
 
-    def __init__(self, dim, L, model, q=0, beta=0.0, seed=1, use_torch=True):
+    def __init__(self, dim, L, model, q=0, beta=0.0, seed=1, use_torch=True, record_bonds=False):
         self._h = C.c_void_p()
         self._ws = None
         self.dim, self.L, self.model, self.q, self.beta, self.seed = dim, L, model, q, beta, seed
@@ -100,6 +101,12 @@ class SwendsenWang:
         else:
             _check(lib().sw_create(C.byref(self._h), dim, L, model, q, float(beta), int(seed)))
         self.N = int(lib().sw_num_sites(self._h))
+        if record_bonds:
+            self.record_bonds(True)
+
+    def record_bonds(self, enable):
+        """Steps after this call also store the bond bytes (needed by bonds())."""
+        _check(lib().sw_set_record_bonds(self._h, int(bool(enable))))
 
     def close(self):
         if self._h:

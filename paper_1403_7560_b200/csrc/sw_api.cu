@@ -23,42 +23,44 @@ int fail(int code, const std::string &msg)
     return code;
 }
 
-// One tile configuration = the three tiled kernels instantiated for it.
+// One tile configuration = the tiled kernels instantiated for it.
 struct TileOps {
-    int tx, ty, tz, nt;
-    size_t smem_bond_label, smem_flip;
+    int tx, ty, tz, nt, nfw, log2ns;
+    size_t smem_bond_label;
     void (*bond_label)(const Params);
     void (*merge)(const Params);
     void (*flip)(const Params);
+    void (*export_labels)(const Params);
+    void (*tile_origin)(const Params);
 };
 
 template <int DIM, int MODEL, int TX, int TY, int TZ>
 TileOps make_ops()
 {
-    using G = TileGeom<DIM, MODEL, TX, TY, TZ>;
+    using G = TileGeom<DIM, TX, TY, TZ>;
     constexpr int NS = G::NS;
-    constexpr int NT = NS / 8 > 1024 ? 1024 : (NS / 8 < 128 ? 128 : NS / 8);
+    constexpr int NT = NS / 16;  // 4 quads = 16 sites per thread
     TileOps o;
-    o.tx = TX; o.ty = TY; o.tz = TZ; o.nt = NT;
-    o.smem_bond_label = G::SMEM_BOND_LABEL;
-    o.smem_flip = G::SMEM_FLIP;
+    o.tx = TX; o.ty = TY; o.tz = TZ; o.nt = NT; o.nfw = G::NFW; o.log2ns = G::LOG2NS;
+    o.smem_bond_label = G::template smem_bond_label<MODEL>();
     o.bond_label = k_bond_label<DIM, MODEL, TX, TY, TZ, NT>;
     o.merge = k_merge<DIM, TX, TY, TZ>;
     o.flip = k_flip<DIM, MODEL, TX, TY, TZ, NT>;
+    o.export_labels = k_export_labels<DIM, TX, TY, TZ>;
+    o.tile_origin = k_tile_origin<TX, TY, TZ>;
     return o;
 }
 
-// Tile menu.  TX is a multiple of 32 (rows are warps); TY, TZ are powers of two <= 32, so they divide
-// every admissible L (multiple of 32); TX > 32 needs L % TX == 0.
+// Tile menu.  Tile sides are powers of two, TX in {32, 64, 128}; every side must divide L.
 template <int MODEL>
 bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
 {
 #define SW_TILE2(X, Y) if (dim == 2 && tx == X && ty == Y) { o = make_ops<2, MODEL, X, Y, 1>(); return true; }
 #define SW_TILE3(X, Y, Z) if (dim == 3 && tx == X && ty == Y && tz == Z) { o = make_ops<3, MODEL, X, Y, Z>(); return true; }
     SW_TILE2(32, 32)
-    SW_TILE2(64, 32)
-    SW_TILE2(128, 16)
+    SW_TILE2(64, 64)
     SW_TILE2(128, 32)
+    SW_TILE2(128, 64)
     SW_TILE3(32, 8, 8)
     SW_TILE3(32, 16, 8)
     SW_TILE3(32, 16, 16)
@@ -75,6 +77,28 @@ bool pick_ops_model(int model, int dim, int tx, int ty, int tz, TileOps &o)
     return pick_ops<XY>(dim, tx, ty, tz, o);
 }
 
+// Default tile of a lattice (SW_B200_TILE=TXxTYxTZ overrides it: a tuning knob).
+void default_tile(int dim, int L, int model, int &tx, int &ty, int &tz)
+{
+    if (dim == 2) {
+        tz = 1;
+        if (L % 128 == 0) { tx = 128; ty = 64; }
+        else if (L % 64 == 0) { tx = 64; ty = 64; }
+        else { tx = 32; ty = 32; }
+    } else {
+        tx = 32; ty = 16; tz = 16;
+        if (model == SW_XY) { ty = 8; tz = 8; }
+    }
+}
+
+int draw_bits(int model, int q)
+{
+    if (model != SW_POTTS) return 1;
+    int b = 1;
+    while ((1 << b) < q) ++b;
+    return b;
+}
+
 size_t align256(size_t v) { return (v + 255) / 256 * 256; }
 
 bool valid_args(int dim, int L, int model, int q, double beta, bool check_beta)
@@ -86,10 +110,12 @@ bool valid_args(int dim, int L, int model, int q, double beta, bool check_beta)
     if (check_beta && !(std::isfinite(beta) && beta >= 0.0)) return false;
     double n = std::pow((double)L, dim);
     if (n > 2147483648.0) return false;
+    // a label word holds (site address << draw bits) | draw
+    if (n * (double)(1u << draw_bits(model, q)) > 4294967296.0) return false;
     return true;
 }
 
-struct Layout { size_t spins, bonds, labels, acc, total; };
+struct Layout { size_t spins, bonds, labels, faces, origin, acc, total; };
 
 Layout layout(int dim, int L, int model)
 {
@@ -100,6 +126,9 @@ Layout layout(int dim, int L, int model)
     l.spins = off; off += align256(N * (model == SW_XY ? 4 : 1));
     l.bonds = off; off += align256(N);
     l.labels = off; off += align256(N * 4);
+    // face words and tile origins: sized for the smallest tile of the menu (1024 sites, <= 18 words)
+    l.faces = off; off += align256((N / 1024) * 18 * 4);
+    l.origin = off; off += align256((N / 1024) * 4);
     l.acc = off; off += align256(sizeof(Acc));
     l.total = off;
     return l;
@@ -116,9 +145,11 @@ struct sw_ctx {
     TileOps ops;
     cudaStream_t stream;
     void *workspace;
+    uint8_t *bonds_mem;
     bool own_workspace, own_stream;
-    bool stepped;      // bonds/labels of a step are available
-    bool labels_flat;
+    bool stepped;      // labels of a step are available
+    bool bonds_valid;  // the last step recorded its bond bytes
+    int record_bonds;
     bool M_fresh;      // acc holds the magnetisation sums of the current configuration
     bool E_fresh;
     int force_phi;
@@ -154,7 +185,7 @@ int check_ctx(sw_ctx *c)
 
 dim3 tile_grid(const sw_ctx *c)
 {
-    return dim3(c->L / c->ops.tx, c->L / c->ops.ty, c->dim == 3 ? c->L / c->ops.tz : 1);
+    return dim3(c->p.ntx, c->p.nty, c->p.ntz);
 }
 
 uint32_t threshold32(double prob)
@@ -212,7 +243,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     if (!out) return fail(SW_EINVAL, "out is NULL");
     *out = nullptr;
     if (!valid_args(dim, L, model, q, beta, true))
-        return fail(SW_EINVAL, "invalid arguments (dim 2|3, L multiple of 32 with L^dim <= 2^31, model, 2<=q<=255, beta>=0)");
+        return fail(SW_EINVAL, "invalid arguments (dim 2|3, L multiple of 32 with L^dim <= 2^31 and L^dim 2^ceil(log2 q) <= 2^32, model, 2<=q<=255, beta>=0)");
     const Layout lay = layout(dim, L, model);
     if (external) {
         if (!workspace || workspace_bytes < lay.total || ((uintptr_t)workspace & 255u))
@@ -239,14 +270,15 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
         e = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking);
         if (e != cudaSuccess) { cudaFree(c->workspace); delete c; return fail(SW_ECUDA, "cudaStreamCreate failed"); }
     }
-    // tile choice: default per dimension, SW_B200_TILE=TXxTYxTZ overrides (tuning knob)
-    int tx = 32, ty = (dim == 2) ? 32 : 8, tz = (dim == 2) ? 1 : 8;
-    if (dim == 2 && L % 128 == 0) { tx = 128; ty = 16; }
+    // tile choice: default per dimension and model, SW_B200_TILE=TXxTYxTZ overrides (tuning knob)
+    int tx, ty, tz;
+    default_tile(dim, L, model, tx, ty, tz);
     if (const char *env = std::getenv("SW_B200_TILE")) {
         int ex = 0, ey = 0, ez = 1;
         if (std::sscanf(env, "%dx%dx%d", &ex, &ey, &ez) >= 2) { tx = ex; ty = ey; tz = (dim == 2) ? 1 : ez; }
     }
-    bool ok = (L % tx == 0) && (L % ty == 0) && (L % tz == 0) && pick_ops_model(model, dim, tx, ty, tz, c->ops);
+    bool ok = tx > 0 && ty > 0 && tz > 0 && (L % tx == 0) && (L % ty == 0) && (L % tz == 0) &&
+              pick_ops_model(model, dim, tx, ty, tz, c->ops);
     if (!ok) {
         tx = 32; ty = (dim == 2) ? 32 : 8; tz = (dim == 2) ? 1 : 8;
         pick_ops_model(model, dim, tx, ty, tz, c->ops);
@@ -254,12 +286,18 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     char *base = (char *)c->workspace;
     Params &p = c->p;
     p.spins = base + lay.spins;
-    p.bonds = (uint8_t *)(base + lay.bonds);
+    p.bonds = nullptr;
+    c->bonds_mem = (uint8_t *)(base + lay.bonds);
     p.labels = (uint32_t *)(base + lay.labels);
+    p.faces = (uint32_t *)(base + lay.faces);
+    p.tile_origin = (uint32_t *)(base + lay.origin);
+    p.labels_out = nullptr;
     p.acc = (Acc *)(base + lay.acc);
+    p.ntx = (uint32_t)(L / c->ops.tx); p.nty = (uint32_t)(L / c->ops.ty);
+    p.ntz = (dim == 3) ? (uint32_t)(L / c->ops.tz) : 1u;
+    p.ntiles = p.ntx * p.nty * p.ntz;
+    p.db = draw_bits(model, q);
     p.L = (uint32_t)L; p.N = (uint32_t)c->N;
-    p.log2L = -1;
-    for (int s = 0; s < 31; ++s) if ((1u << s) == (uint32_t)L) p.log2L = s;
     p.k0 = (uint32_t)(seed & 0xffffffffu); p.k1 = (uint32_t)(seed >> 32);
     p.t_lo = p.t_hi = 0;
     // PAPER.md:96 (garbled "p = 1 e^{2J/T}"): Ising p = 1 - exp(-2 beta); PAPER.md:152 + Eq. 2: Potts
@@ -283,8 +321,9 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     };
     e = cudaFuncSetAttribute(c->ops.bond_label, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ops.smem_bond_label);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_bond_label)");
-    e = cudaFuncSetAttribute(c->ops.flip, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ops.smem_flip);
-    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_flip)");
+    c->ops.tile_origin<<<(p.ntiles + 255) / 256, 256, 0, c->stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return bail(e, "k_tile_origin launch");
     e = cudaMemsetAsync(p.acc, 0, sizeof(Acc), c->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync");
     if (model == SW_ISING) launch_init<ISING>(c);
@@ -292,7 +331,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     else launch_init<XY>(c);
     e = cudaGetLastError();
     if (e != cudaSuccess) return bail(e, "k_init launch");
-    c->stepped = false; c->labels_flat = false; c->M_fresh = false; c->E_fresh = false;
+    c->stepped = false; c->bonds_valid = false; c->record_bonds = 0; c->M_fresh = false; c->E_fresh = false;
     *out = c;
     return SW_OK;
 }
@@ -326,9 +365,10 @@ int sw_step(sw_ctx *c, int n)
     if (rc) return rc;
     if (n < 0) return fail(SW_EINVAL, "n < 0");
     const dim3 grid = tile_grid(c);
-    const uint32_t slots = (uint32_t)(c->N / c->ops.tx + c->N / c->ops.ty + (c->dim == 3 ? c->N / c->ops.tz : 0));
+    const uint32_t slots = c->p.ntiles * 32u * (uint32_t)c->ops.nfw;
     for (int s = 0; s < n; ++s) {
         Params &p = c->p;
+        p.bonds = c->record_bonds ? c->bonds_mem : nullptr;
         p.t_lo = (uint32_t)(c->t & 0xffffffffu);
         p.t_hi = (uint32_t)(c->t >> 32);
         if (c->model == SW_XY) {
@@ -342,13 +382,18 @@ int sw_step(sw_ctx *c, int n)
             p.ry = c->ry = (float)std::sin(phi);
             p.crefl = c->crefl = (float)std::fmod(2.0 * phi + two_pi / 2.0, two_pi);
         }
-        if (p.counting) SW_CUDA(c, cudaMemsetAsync(p.acc->stats, 0, sizeof(p.acc->stats), c->stream));
+        if (p.counting) {
+            SW_CUDA(c, cudaMemsetAsync(p.acc->stats, 0, sizeof(p.acc->stats), c->stream));
+            const unsigned long long examined = (unsigned long long)c->N / c->ops.tx + c->N / c->ops.ty +
+                                                (c->dim == 3 ? c->N / c->ops.tz : 0);
+            SW_CUDA(c, cudaMemcpyAsync(&p.acc->stats[0], &examined, 8, cudaMemcpyHostToDevice, c->stream));
+        }
         if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[0], c->stream));
         c->ops.bond_label<<<grid, c->ops.nt, c->ops.smem_bond_label, c->stream>>>(p);
         if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[1], c->stream));
         c->ops.merge<<<(slots + 255) / 256, 256, 0, c->stream>>>(p);
         if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[2], c->stream));
-        c->ops.flip<<<grid, c->ops.nt, c->ops.smem_flip, c->stream>>>(p);
+        c->ops.flip<<<grid, c->ops.nt, 0, c->stream>>>(p);
         if (c->timing) {
             SW_CUDA(c, cudaEventRecord(c->ev[3], c->stream));
             SW_CUDA(c, cudaEventSynchronize(c->ev[3]));
@@ -363,7 +408,9 @@ int sw_step(sw_ctx *c, int n)
     }
     if (n > 0) {
         SW_CUDA(c, cudaGetLastError());
-        c->stepped = true; c->labels_flat = false; c->M_fresh = true; c->E_fresh = false;
+        c->stepped = true; c->bonds_valid = c->record_bonds != 0;
+        c->M_fresh = (c->model != SW_XY);  // XY: the vector magnetisation is summed on request
+        c->E_fresh = false;
     }
     return SW_OK;
 }
@@ -437,7 +484,7 @@ int sw_set_spins(sw_ctx *c, const void *src, size_t bytes, uint64_t step)
     SW_CUDA(c, cudaMemcpyAsync(c->p.spins, src, want, cudaMemcpyHostToDevice, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
     c->t = step;
-    c->stepped = false; c->labels_flat = false; c->M_fresh = false; c->E_fresh = false;
+    c->stepped = false; c->bonds_valid = false; c->M_fresh = false; c->E_fresh = false;
     return SW_OK;
 }
 
@@ -446,8 +493,9 @@ int sw_get_bonds(sw_ctx *c, uint8_t *dst, size_t bytes)
     int rc = check_ctx(c);
     if (rc) return rc;
     if (!c->stepped) return fail(SW_ESTATE, "no step since create / sw_set_spins");
+    if (!c->bonds_valid) return fail(SW_ESTATE, "the last step did not record its bonds (sw_set_record_bonds)");
     if (!dst || bytes != c->N) return fail(SW_EINVAL, "sw_get_bonds: buffer must hold exactly N bytes");
-    SW_CUDA(c, cudaMemcpyAsync(dst, c->p.bonds, c->N, cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaMemcpyAsync(dst, c->bonds_mem, c->N, cudaMemcpyDeviceToHost, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
     return SW_OK;
 }
@@ -458,13 +506,19 @@ int sw_get_labels(sw_ctx *c, uint32_t *dst, size_t bytes)
     if (rc) return rc;
     if (!c->stepped) return fail(SW_ESTATE, "no step since create / sw_set_spins");
     if (!dst || bytes != c->N * 4) return fail(SW_EINVAL, "sw_get_labels: buffer must hold exactly N uint32");
-    if (!c->labels_flat) {
-        k_flatten<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->p);
-        SW_CUDA(c, cudaGetLastError());
-        c->labels_flat = true;
-    }
-    SW_CUDA(c, cudaMemcpyAsync(dst, c->p.labels, c->N * 4, cudaMemcpyDeviceToHost, c->stream));
-    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    // canonical labels (minimum linear site index, linear order) are made on request, in scratch
+    // device memory that lives only for this call: the step itself never needs them
+    uint32_t *out = nullptr;
+    cudaError_t e = cudaMalloc(&out, c->N * 4);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SW_ENOMEM, "sw_get_labels: cudaMalloc of the export buffer failed"); }
+    Params q = c->p;
+    q.labels_out = out;
+    c->ops.export_labels<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(q);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dst, out, c->N * 4, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(out);
+    if (e != cudaSuccess) return cuda_fail(c, e, "sw_get_labels");
     return SW_OK;
 }
 
@@ -504,6 +558,14 @@ int sw_force_xy_phi(sw_ctx *c, int enable, double phi)
     if (rc) return rc;
     if (c->model != SW_XY) return fail(SW_EINVAL, "not an XY context");
     c->force_phi = enable; c->forced_phi = phi;
+    return SW_OK;
+}
+
+int sw_set_record_bonds(sw_ctx *c, int enable)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    c->record_bonds = enable ? 1 : 0;
     return SW_OK;
 }
 

@@ -3,12 +3,22 @@
 //
 // Kernels of one step t:
 //   k_bond_label  (1) bond activation fused with (2a) tile-local cluster labelling in
-//                 shared memory: warp-ballot run detection along x + atomicMin union-find;
-//   k_merge       (2b) global atomicMin union-find over the active bonds that cross tile faces
-//                 (incl. the periodic wrap), PAPER.md:97, 100-104;
-//   k_flip        (2c) root chase (flatten) fused with (3) the per-cluster draw / XY reflection
+//                 shared memory.  A thread owns "quads" of 4 consecutive sites along x (one 32-bit
+//                 spin word); x-connectivity is resolved with two warp ballots, y/z bonds inside the
+//                 tile by an atomicMin union-find in shared memory;
+//   k_merge       (2b) global lock-free union-find (atomicCAS, min linear index wins) over the active
+//                 bonds that cross tile faces incl. the periodic wrap;
+//   k_flip        (2c) root chase fused with (3) the per-cluster new value / XY reflection
 //                  and the magnetisation sums of PAPER.md:142-157;
 //   k_measure     energy (Eq. 1-3) and magnetisation (Eq. 4, 5) of the current configuration.
+//
+// Label array (HBM), one 32-bit word per site, TILE-MAJOR: the word of the site with tile-local
+// index li = lx + TX (ly + TY lz) in tile T lives at address a = T * NS + li, and holds
+//     (parent address << DB) | (the site's own cluster draw, DB bits: word 3 of its Philox call).
+// A site is a root iff parent address == own address.  Hooking always puts the root with the larger
+// LINEAR site index under the one with the smaller, so the final root of a cluster is its minimum
+// linear site index (what label equivalence with atomicMin from label = index converges to,
+// PAPER.md:102), and the cluster's new value is simply the draw field of the root's word.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -18,6 +28,12 @@ namespace swk {
 enum { ISING = 0, POTTS = 1, XY = 2 };
 constexpr uint32_t DOM_SITE = 0u, DOM_INIT = 2u, DOM_XYDIR = 3u;
 constexpr uint32_t FULL = 0xffffffffu;
+#ifndef SW_BL_THREADS_PER_SM
+#define SW_BL_THREADS_PER_SM 1024  // resident threads per SM k_bond_label is compiled for (register cap)
+#endif
+#ifndef SW_BL_JUMPS
+#define SW_BL_JUMPS 2  // pointer-jumping rounds over the tile-local forest before it is stored
+#endif
 
 // Device accumulators of the observables and the labelling counters.
 struct Acc {
@@ -30,16 +46,20 @@ struct Acc {
 };
 
 struct Params {
-    void *spins;       // int8 (Ising) | uint8 (Potts) | float (XY angle), N elements
-    uint8_t *bonds;    // N bytes, bit k = bond i -> i + e_k
-    uint32_t *labels;  // N parent pointers, label[i] <= i, roots have label[i] == i
+    void *spins;            // int8 (Ising) | uint8 (Potts) | float (XY angle), N elements, linear order
+    uint8_t *bonds;         // N bytes, bit k = bond i -> i + e_k, linear order; NULL = not recorded
+    uint32_t *labels;       // N packed parent words, tile-major (see above)
+    uint32_t *faces;        // per tile NFW words: active bonds through the +x, +y, +z tile faces
+    uint32_t *tile_origin;  // per tile: linear index of its first site
+    uint32_t *labels_out;   // k_export_labels: N canonical labels (minimum linear index), linear order
     Acc *acc;
     uint32_t L, N;
-    int log2L;         // >= 0 if L is a power of two, else -1
+    uint32_t ntx, nty, ntz, ntiles;
     uint32_t k0, k1;   // Philox key = (seed low, seed high)
     uint32_t t_lo, t_hi;
     uint32_t P32;      // Ising/Potts: bond active iff word < P32
     int q;
+    int db;            // draw bits in a label word: 1 (Ising, XY), ceil(log2 q) (Potts)
     float rx, ry, crefl, m2beta;  // XY: direction, reflection constant, -2 beta
     int counting;
 };
@@ -66,31 +86,60 @@ __host__ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1
 
 __device__ __forceinline__ void decode(const Params &p, uint32_t i, uint32_t &x, uint32_t &y, uint32_t &z)
 {
-    if (p.log2L >= 0) {
-        x = i & (p.L - 1u);
-        y = (i >> p.log2L) & (p.L - 1u);
-        z = i >> (2 * p.log2L);
-    } else {
-        x = i % p.L;
-        const uint32_t r = i / p.L;
-        y = r % p.L;
-        z = r / p.L;
-    }
+    x = i % p.L;
+    const uint32_t r = i / p.L;
+    y = r % p.L;
+    z = r / p.L;
 }
 
-template <int MODEL> struct ValT { using type = uint8_t; };
-template <> struct ValT<XY> { using type = float; };
+constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v / 2); }
+
+// Geometry of a TX x TY x TZ tile (powers of two; TX a multiple of 32).
+template <int DIM, int TX, int TY, int TZ>
+struct TileGeom {
+    static constexpr int NS = TX * TY * TZ;
+    static constexpr int LOG2NS = ilog2(NS);
+    static_assert((1 << LOG2NS) == NS, "tile sizes are powers of two");
+    static_assert(TX % 32 == 0 && TX <= 128, "a tile row is 8, 16 or 32 quads");
+    static_assert(DIM == 3 || TZ == 1, "2D tiles have TZ = 1");
+    // face bit fields: +x face TY*TZ bonds, +y face TX*TZ bonds, +z face TX*TY bonds
+    static constexpr int FXB = TY * TZ, FYB = TX * TZ, FZB = (DIM == 3) ? TX * TY : 0;
+    static constexpr int FXW = (FXB + 31) / 32, FYW = (FYB + 31) / 32, FZW = (FZB + 31) / 32;
+    static constexpr int NFW = FXW + FYW + FZW;
+    static constexpr int NFWP = (NFW + 3) / 4 * 4;  // padded: what follows in smem stays 16-byte aligned
+    static constexpr int NHALO = FXB + FYB + FZB;  // XY: projections of the three plus-faces
+    template <int MODEL> static constexpr size_t smem_bond_label()
+    {
+        return (size_t)NS * 4 + (size_t)NFWP * 4 + (MODEL == XY ? ((size_t)NS + NHALO) * 4 : 0);
+    }
+};
+
+// 4-bit mask of the byte positions where a and b hold equal bytes.
+__device__ __forceinline__ uint32_t eq4(uint32_t a, uint32_t b)
+{
+    const uint32_t t = a ^ b;
+    const uint32_t z = ~(((t & 0x7f7f7f7fu) + 0x7f7f7f7fu) | t | 0x7f7f7f7fu);  // 0x80 per zero byte
+    return (((z >> 7) * 0x00204081u) >> 21) & 0xfu;
+}
+// bit s of a nibble -> bit 0 of byte s
+__device__ __forceinline__ uint32_t spread4(uint32_t n) { return (n * 0x00204081u) & 0x01010101u; }
 
 // ------------------------------------------------------------------------------------------------
 // Shared-memory union-find (min-index roots).  Every link hangs the larger root under the smaller
 // one, so the root of a finished tree is the minimum index of its set whatever the order in which
-// concurrent unions land (the paper's analogue: atomicMin on labels initialised to the site index,
-// PAPER.md:102).
+// concurrent unions land.  Tile-local indices are monotone in the linear site index.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t find_s(volatile uint32_t *lab, uint32_t x)
 {
-    uint32_t n;
-    while ((n = lab[x]) != x) x = n;
+    // path splitting: every node passed is re-pointed to its grandparent (plain stores of valid
+    // ancestors; a root is never written here, so the atomicMin hooks are not disturbed)
+    uint32_t p = lab[x];
+    while (p != x) {
+        const uint32_t gp = lab[p];
+        if (gp != p) lab[x] = gp;
+        x = p;
+        p = gp;
+    }
     return x;
 }
 
@@ -104,23 +153,6 @@ __device__ __forceinline__ void union_s(uint32_t *lab, uint32_t a, uint32_t b)
         const uint32_t old = atomicMin(&lab[a], b);
         if (old == a) return;  // a was a root and now hangs under b
         a = old;               // a had been linked meanwhile: go on with (old parent, b)
-    }
-}
-
-// Global union-find over the label array.  Loads bypass L1 (volatile) because other CTAs update
-// parents concurrently; every update is an atomicMin, so parents only ever decrease.
-__device__ __forceinline__ uint32_t find_g(uint32_t *lab, uint32_t x, unsigned &hops)
-{
-    volatile uint32_t *vl = lab;
-    for (;;) {
-        const uint32_t p = vl[x];
-        if (p == x) return x;
-        const uint32_t gp = vl[p];
-        ++hops;
-        if (gp == p) return p;
-        atomicMin(&lab[x], gp);  // path halving; result unused -> RED
-        x = gp;
-        ++hops;
     }
 }
 
@@ -138,385 +170,463 @@ __global__ void __launch_bounds__(256) k_init(const Params p)
     else ((float *)p.spins)[i] = (float)(w >> 8) * (float)(6.283185307179586476925286766559 / 16777216.0);
 }
 
-// ------------------------------------------------------------------------------------------------
-// k_bond_label: one CTA per TX x TY x TZ tile.
-//   (XY only) stage the projections a_i = r . s_i of the tile and its +x/+y/+z faces in smem
-//   rows    one warp per row of 32 sites along x: Philox(site, t) -> bond bits; the ballot of the
-//           x-bond bits gives every lane the start of its run, so x-connectivity costs no union;
-//           active y/z bonds inside the tile are compacted into a work list (ballot + popc)
-//   unions  the work list is processed densely, one bond per thread: atomicMin union-find in smem
-//   flatten label[i] = global index of the tile-local root
-// Local index order (lx fastest, then ly, lz) is monotone in the global index inside a tile, so the
-// tile-local minimum is the global minimum over the tile's part of the cluster.
-// ------------------------------------------------------------------------------------------------
-template <int DIM, int MODEL, int TX, int TY, int TZ>
-struct TileGeom {
-    static constexpr int SX = TX + 1, SY = TY + 1, SZ = (DIM == 3) ? TZ + 1 : 1;
-    static constexpr int NS = TX * TY * TZ;
-    static_assert(NS <= 8192, "work-list entries keep the local index in 13 bits");
-    static constexpr int NSTAGE = (MODEL == XY) ? SX * SY * SZ : 0;
-    static constexpr int NWORK = 2 * NS + NS / 32;  // every y/z bond of the tile + the x seams
-    static constexpr size_t VAL_BYTES = ((size_t)NSTAGE * 4 + 15) / 16 * 16;
-    static constexpr size_t OFF_LAB = VAL_BYTES;
-    static constexpr size_t OFF_WORK = OFF_LAB + (size_t)NS * 4;
-    static constexpr size_t SMEM_BOND_LABEL = OFF_WORK + (size_t)NWORK * 2;
-    static constexpr size_t SMEM_FLIP = (size_t)NS * 4 + (size_t)NS + (size_t)NS * 2;
-};
-
-template <int DIM, int MODEL, int TX, int TY, int TZ, int NT>
-__global__ void __launch_bounds__(NT) k_bond_label(const Params p)
+// tile_origin[T] = linear index of the first site of tile T (T = tx + ntx (ty + nty tz)).
+template <int TX, int TY, int TZ>
+__global__ void __launch_bounds__(256) k_tile_origin(const Params p)
 {
-    static_assert(TX % 32 == 0, "rows are warps");
-    using G = TileGeom<DIM, MODEL, TX, TY, TZ>;
-    constexpr int SX = G::SX, SY = G::SY, SZ = G::SZ, NS = G::NS;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float *val_s = reinterpret_cast<float *>(smem_raw);
-    uint32_t *lab_s = reinterpret_cast<uint32_t *>(smem_raw + G::OFF_LAB);
-    uint16_t *work_s = reinterpret_cast<uint16_t *>(smem_raw + G::OFF_WORK);
-    __shared__ int count_s;
+    const uint32_t T = blockIdx.x * 256u + threadIdx.x;
+    if (T >= p.ntiles) return;
+    const uint32_t tx = T % p.ntx, r = T / p.ntx, ty = r % p.nty, tz = r / p.nty;
+    p.tile_origin[T] = tx * TX + p.L * (ty * TY + p.L * (tz * TZ));
+}
+
+// ------------------------------------------------------------------------------------------------
+// k_bond_label: one CTA per tile, QPT quads per thread.
+//   phase 0 (XY)  projections a_i = r . s_i of the tile and its three plus-faces into smem
+//   phase 1       per quad: spins of the quad and of its +x/+y/+z neighbours, one Philox call per
+//                 site, bond nibbles; two ballots give every site the start of its
+//                 x-run; label_s[site] = run start; face bonds -> face bit words
+//   phase 2       every thread walks the set bits of its y/z work mask: atomicMin union in smem
+//   phase 3       label word = (address of the tile-local root << DB) | own draw, 16-byte stores
+// ------------------------------------------------------------------------------------------------
+template <int DIM, int MODEL, int TX, int TY, int TZ, int NT>
+__global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(const Params p)
+{
+    using G = TileGeom<DIM, TX, TY, TZ>;
+    constexpr int NS = G::NS, NQ = NS / 4, QPT = NQ / NT, LPR = TX / 4;
+    constexpr int WB = (DIM == 3) ? 8 : 4;  // work bits per quad: 4 y bonds (+ 4 z bonds)
+    static_assert(NQ % NT == 0 && NT % 32 == 0, "whole quads per thread, whole rows per warp");
+    static_assert(QPT * WB <= 32, "the work mask of a thread is one 32-bit word");
+    extern __shared__ __align__(16) uint32_t smem_u32[];
+    uint32_t *lab_s = smem_u32;
+    uint32_t *face_s = smem_u32 + NS;
+    float *val_s = reinterpret_cast<float *>(smem_u32 + NS + G::NFWP);  // XY only: NS + NHALO floats
 
     const uint32_t L = p.L;
     const uint32_t x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = (DIM == 3) ? blockIdx.z * TZ : 0u;
-    const int tid = threadIdx.x;
-    constexpr int ROWS = NS / 32, NW = NT / 32;
-    const int lane = tid & 31, warp = tid >> 5;
+    const uint32_t tile = blockIdx.x + p.ntx * (blockIdx.y + p.nty * blockIdx.z);
+    const uint32_t tile_base = tile << G::LOG2NS;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const uint32_t LL = L * L;
 
-    if (tid == 0) count_s = 0;
+    if (tid < G::NFW) face_s[tid] = 0u;
+
     if (MODEL == XY) {
-        // a_i = r . s_i for the tile and its three plus-faces, one staged row per warp
-        for (int r = warp; r < SY * SZ; r += NW) {
-            const int ly = r % SY, lz = r / SY;
-            const bool face = (ly == TY) || (DIM == 3 && lz == TZ);
-            if (ly == TY && DIM == 3 && lz == TZ) continue;
-            uint32_t gy = y0 + ly, gz = z0 + lz;
+        // a_i = r . s_i: interior, then the +x, +y, +z faces (periodic wrap)
+        const float *th = (const float *)p.spins;
+#pragma unroll
+        for (int j = 0; j < QPT; ++j) {
+            const int li = (tid + j * NT) * 4;
+            const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
+            const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
+            const float4 t4 = *reinterpret_cast<const float4 *>(th + g);
+            float4 a;
+            float sn, cs;
+            sincosf(t4.x, &sn, &cs); a.x = p.rx * cs + p.ry * sn;
+            sincosf(t4.y, &sn, &cs); a.y = p.rx * cs + p.ry * sn;
+            sincosf(t4.z, &sn, &cs); a.z = p.rx * cs + p.ry * sn;
+            sincosf(t4.w, &sn, &cs); a.w = p.rx * cs + p.ry * sn;
+            *reinterpret_cast<float4 *>(val_s + li) = a;
+        }
+        for (int h = tid; h < G::NHALO; h += NT) {
+            uint32_t gx, gy, gz;
+            if (h < G::FXB) {
+                gx = x0 + TX; gy = y0 + h % TY; gz = z0 + h / TY;
+            } else if (h < G::FXB + G::FYB) {
+                const int k = h - G::FXB;
+                gx = x0 + k % TX; gy = y0 + TY; gz = z0 + k / TX;
+            } else {
+                const int k = h - G::FXB - G::FYB;
+                gx = x0 + k % TX; gy = y0 + k / TX; gz = z0 + TZ;
+            }
+            if (gx == L) gx = 0;
             if (gy == L) gy = 0;
             if (DIM == 3 && gz == L) gz = 0;
-            const uint32_t rowbase = L * (gy + L * gz);
-            for (int lx = lane; lx < SX; lx += 32) {
-                if (face && lx == TX) continue;
-                uint32_t gx = x0 + lx;
-                if (gx == L) gx = 0;
-                float sn, cs;
-                sincosf(((const float *)p.spins)[rowbase + gx], &sn, &cs);
-                val_s[(lz * SY + ly) * SX + lx] = p.rx * cs + p.ry * sn;
-            }
+            float sn, cs;
+            sincosf(th[gx + L * (gy + L * gz)], &sn, &cs);
+            val_s[NS + h] = p.rx * cs + p.ry * sn;
         }
     }
     __syncthreads();
 
-    for (int row = warp; row < ROWS; row += NW) {
-        const int li = row * 32 + lane;
+    uint32_t bnd[QPT];   // per quad: bits 0-3 x bonds, 4-7 y bonds, 8-11 z bonds
+    uint32_t drw[QPT];   // per quad: the four draws, DB bits each (site s at bit s * db)
+    uint32_t work = 0u;  // per quad WB bits: y (and z) bonds that stay inside the tile
+    const int db = (MODEL == POTTS) ? p.db : 1;
+
+#pragma unroll
+    for (int j = 0; j < QPT; ++j) {
+        const int li = (tid + j * NT) * 4;
         const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
         const uint32_t gx = x0 + lx, gy = y0 + ly, gz = z0 + lz;
         const uint32_t g = gx + L * (gy + L * gz);
-        const uint4 w = philox4x32_10(g, p.t_lo, p.t_hi, DOM_SITE, p.k0, p.k1);
-        uint32_t b = 0;
+        const bool rowend = (lane & (LPR - 1)) == LPR - 1;
+        uint4 w[4];
+#pragma unroll
+        for (int s = 0; s < 4; ++s) w[s] = philox4x32_10(g + s, p.t_lo, p.t_hi, DOM_SITE, p.k0, p.k1);
+        uint32_t bxn, byn, bzn = 0u, d;
         if (MODEL == XY) {
             // Wolff embedding: aligned iff a_i a_j > 0, p = 1 - exp(-2 beta a_i a_j)
-            const int si = (lz * SY + ly) * SX + lx;
             const float scale = 5.9604644775390625e-8f;  // 2^-24
-            const float v = val_s[si];
-            const float px = v * val_s[si + 1];
-            const float py = v * val_s[si + SX];
-            if (px > 0.f && (float)(w.x >> 8) * scale < -expm1f(p.m2beta * px)) b |= 1u;
-            if (py > 0.f && (float)(w.y >> 8) * scale < -expm1f(p.m2beta * py)) b |= 2u;
-            if (DIM == 3) {
-                const float pz = v * val_s[si + SX * SY];
-                if (pz > 0.f && (float)(w.z >> 8) * scale < -expm1f(p.m2beta * pz)) b |= 4u;
+            const float4 a = *reinterpret_cast<const float4 *>(val_s + li);
+            const float ax3 = (lx + 4 < TX) ? val_s[li + 4] : val_s[NS + ly + TY * lz];
+            const float4 ay = (ly + 1 < TY) ? *reinterpret_cast<const float4 *>(val_s + li + TX)
+                                            : *reinterpret_cast<const float4 *>(val_s + NS + G::FXB + lx + TX * lz);
+            const float av[4] = {a.x, a.y, a.z, a.w};
+            const float axv[4] = {a.y, a.z, a.w, ax3};
+            const float ayv[4] = {ay.x, ay.y, ay.z, ay.w};
+            bxn = byn = 0u;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const float px = av[s] * axv[s], py = av[s] * ayv[s];
+                if (px > 0.f && (float)(w[s].x >> 8) * scale < -expm1f(p.m2beta * px)) bxn |= 1u << s;
+                if (py > 0.f && (float)(w[s].y >> 8) * scale < -expm1f(p.m2beta * py)) byn |= 1u << s;
             }
+            if (DIM == 3) {
+                const float4 az = (lz + 1 < TZ) ? *reinterpret_cast<const float4 *>(val_s + li + TX * TY)
+                                                : *reinterpret_cast<const float4 *>(val_s + NS + G::FXB + G::FYB + lx + TX * ly);
+                const float azv[4] = {az.x, az.y, az.z, az.w};
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    const float pz = av[s] * azv[s];
+                    if (pz > 0.f && (float)(w[s].z >> 8) * scale < -expm1f(p.m2beta * pz)) bzn |= 1u << s;
+                }
+            }
+            d = (w[0].w >> 31) | ((w[1].w >> 31) << 1) | ((w[2].w >> 31) << 2) | ((w[3].w >> 31) << 3);
         } else {
-            // a bond between equal neighbours is active with probability p.
-            // Spins straight from global memory (the +y/+z rows hit L1: other warps load them as theirs).
+            // a bond between equal neighbours is active with probability p (word < P32).
             const uint8_t *sp = (const uint8_t *)p.spins;
-            const uint32_t v = sp[g];
-            uint32_t vx = __shfl_down_sync(FULL, v, 1);
-            if (lane == 31) vx = sp[(gx + 1 == L) ? g - (L - 1) : g + 1];
-            const uint32_t vy = sp[(gy + 1 == L) ? g - L * (L - 1) : g + L];
-            if (v == vx && w.x < p.P32) b |= 1u;
-            if (v == vy && w.y < p.P32) b |= 2u;
+            const uint32_t own = *reinterpret_cast<const uint32_t *>(sp + g);
+            const uint32_t up = *reinterpret_cast<const uint32_t *>(sp + ((gy + 1 == L) ? g - L * (L - 1) : g + L));
+            uint32_t nb = __shfl_down_sync(FULL, own, 1);
+            if (rowend) nb = sp[(gx + 4 == L) ? g + 4 - L : g + 4];
+            const uint32_t P = p.P32;
+            bxn = eq4(own, __funnelshift_r(own, nb, 8)) &
+                  ((w[0].x < P) | ((w[1].x < P) << 1) | ((w[2].x < P) << 2) | ((w[3].x < P) << 3));
+            byn = eq4(own, up) & ((w[0].y < P) | ((w[1].y < P) << 1) | ((w[2].y < P) << 2) | ((w[3].y < P) << 3));
             if (DIM == 3) {
-                const uint32_t LL = L * L;
-                const uint32_t vz = sp[(gz + 1 == L) ? g - LL * (L - 1) : g + LL];
-                if (v == vz && w.z < p.P32) b |= 4u;
+                const uint32_t fr = *reinterpret_cast<const uint32_t *>(sp + ((gz + 1 == L) ? g - LL * (L - 1) : g + LL));
+                bzn = eq4(own, fr) & ((w[0].z < P) | ((w[1].z < P) << 1) | ((w[2].z < P) << 2) | ((w[3].z < P) << 3));
+            }
+            if (MODEL == POTTS) {
+                const unsigned qq = (unsigned)p.q;
+                d = 0u;
+#pragma unroll
+                for (int s = 0; s < 4; ++s) d |= (uint32_t)(((unsigned long long)w[s].w * qq) >> 32) << (s * db);
+            } else {
+                d = (w[0].w >> 31) | ((w[1].w >> 31) << 1) | ((w[2].w >> 31) << 2) | ((w[3].w >> 31) << 3);
             }
         }
-        p.bonds[g] = (uint8_t)b;
-        const uint32_t xm = __ballot_sync(FULL, b & 1u);
+        bnd[j] = bxn | (byn << 4) | (bzn << 8);
+        drw[j] = d;
+
+        // x-runs: link = my last site is bonded to the next quad of the row, thru = no break inside
+        const uint32_t Lk = __ballot_sync(FULL, (bxn & 8u) && !rowend);
+        const uint32_t Th = __ballot_sync(FULL, (bxn & 7u) == 7u);
+        const uint32_t E = Th & (Lk << 1);                 // entering quad c from the right leaves it to the left
+        const uint32_t z3 = ~bxn & 7u;
+        const int tails = z3 ? 32 - __clz(z3) : 0;         // first site of the run that reaches my site 3
         const uint32_t below = (1u << lane) - 1u;
-        const uint32_t zeros = ~xm & below;  // lanes below me whose +x bond is off
-        const int start = zeros ? 32 - __clz(zeros) : 0;
-        lab_s[li] = (uint32_t)(row * 32 + start);
-        // compact the bonds that need a union: +y / +z inside the tile, +x across a 32-lane seam
-        const bool wy = (b & 2u) && ly < TY - 1;
-        const bool wz = DIM == 3 && (b & 4u) && lz < TZ - 1;
-        const bool wx = TX > 32 && (b & 1u) && lane == 31 && lx < TX - 1;
-        const uint32_t my = __ballot_sync(FULL, wy), mz = __ballot_sync(FULL, wz);
-        const int nx = (TX > 32) ? (int)((__ballot_sync(FULL, wx) >> 31) & 1u) : 0;
-        const int ny = __popc(my), nz = __popc(mz);
-        int base = 0;
-        if (lane == 0 && ny + nz + nx > 0) base = atomicAdd(&count_s, ny + nz + nx);
-        base = __shfl_sync(FULL, base, 0);
-        if (wy) work_s[base + __popc(my & below)] = (uint16_t)(li | (1u << 13));
-        if (wz) work_s[base + ny + __popc(mz & below)] = (uint16_t)(li | (2u << 13));
-        if (wx) work_s[base + ny + nz] = (uint16_t)li;
+        const bool linked_prev = (Lk << 1) >> lane & 1u;
+        const uint32_t zE = ~E & below;
+        const int q0 = linked_prev ? 31 - __clz(zE) : lane;  // quad in which the run of my site 0 starts
+        const int tq = __shfl_sync(FULL, tails, q0);
+        const uint32_t s0 = linked_prev ? (uint32_t)(li - 4 * (lane - q0) + tq) : (uint32_t)li;
+        const uint32_t s1 = (bxn & 1u) ? s0 : (uint32_t)li + 1u;
+        const uint32_t s2 = (bxn & 2u) ? s1 : (uint32_t)li + 2u;
+        const uint32_t s3 = (bxn & 4u) ? s2 : (uint32_t)li + 3u;
+        *reinterpret_cast<uint4 *>(lab_s + li) = make_uint4(s0, s1, s2, s3);
+
+        // bonds through the tile faces (incl. the periodic wrap) go to the global merge
+        if (rowend && (bxn & 8u)) {
+            const int r = ly + TY * lz;
+            atomicOr(&face_s[r >> 5], 1u << (r & 31));
+        }
+        if (ly == TY - 1 && byn) {
+            const int b = lx + TX * lz;
+            atomicOr(&face_s[G::FXW + (b >> 5)], byn << (b & 31));
+        }
+        if (DIM == 3 && lz == TZ - 1 && bzn) {
+            const int b = lx + TX * ly;
+            atomicOr(&face_s[G::FXW + G::FYW + (b >> 5)], bzn << (b & 31));
+        }
+        uint32_t wk = (ly < TY - 1) ? byn : 0u;
+        if (DIM == 3 && lz < TZ - 1) wk |= bzn << 4;
+        work |= wk << (j * WB);
     }
     __syncthreads();
 
-    const int nwork = count_s;
-    for (int e0 = 0; e0 < nwork; e0 += NT) {
-        const int e = e0 + tid;
-        if (e < nwork) {
-            const uint32_t wk = work_s[e];
-            const uint32_t a = wk & 0x1fffu, d = wk >> 13;
-            union_s(lab_s, a, a + (d == 0 ? 1u : (d == 1 ? (uint32_t)TX : (uint32_t)(TX * TY))));
+    // warp-uniform trip count + __syncwarp: lanes whose union ends early wait for the others instead
+    // of drifting into later iterations on their own (that would serialise the warp)
+    while (__any_sync(FULL, work != 0u)) {
+        if (work) {
+            const int k = __ffs(work) - 1;
+            work &= work - 1u;
+            const int jq = k / WB, r = k % WB;
+            const uint32_t a = (uint32_t)((tid + jq * NT) * 4 + (r & 3));
+            union_s(lab_s, a, a + ((r & 4) ? (uint32_t)(TX * TY) : (uint32_t)TX));
         }
         __syncwarp();
     }
     __syncthreads();
 
-    for (int row = warp; row < ROWS; row += NW) {
-        const int li = row * 32 + lane;
-        const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
-        const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
-        const uint32_t r = find_s(lab_s, li);
-        __syncwarp();
-        const int rx = r % TX, ry = (r / TX) % TY, rz = r / (TX * TY);
-        p.labels[g] = (x0 + rx) + L * ((y0 + ry) + L * (z0 + rz));
+    if (tid < G::NFW) p.faces[tile * G::NFW + tid] = face_s[tid];
+    // phase 3: no unions any more, the forest is static.  JUMPS rounds of pointer jumping (uniform
+    // work, no divergence; a thread only rewrites the entries of its own sites, and whatever another
+    // thread reads is a valid ancestor), then the parent is stored as it stands: k_merge and k_flip
+    // follow whatever is left of the chain through L1/L2.
+    volatile uint32_t *vlab = lab_s;
+#pragma unroll
+    for (int j = 0; j < QPT; ++j) {
+        const int li = (tid + j * NT) * 4;
+        uint4 r = *reinterpret_cast<const uint4 *>(lab_s + li);
+#pragma unroll
+        for (int k = 0; k < SW_BL_JUMPS; ++k) {
+            r.x = vlab[r.x]; r.y = vlab[r.y]; r.z = vlab[r.z]; r.w = vlab[r.w];
+            if (k + 1 < SW_BL_JUMPS) *reinterpret_cast<uint4 *>(lab_s + li) = r;
+        }
+        const uint32_t dm = (1u << db) - 1u, d = drw[j];
+        uint4 o;
+        o.x = ((tile_base + r.x) << db) | (d & dm);
+        o.y = ((tile_base + r.y) << db) | ((d >> db) & dm);
+        o.z = ((tile_base + r.z) << db) | ((d >> (2 * db)) & dm);
+        o.w = ((tile_base + r.w) << db) | ((d >> (3 * db)) & dm);
+        *reinterpret_cast<uint4 *>(p.labels + tile_base + li) = o;
+        if (p.bonds) {
+            const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
+            const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
+            *reinterpret_cast<uint32_t *>(p.bonds + g) =
+                spread4(bnd[j] & 0xfu) | (spread4((bnd[j] >> 4) & 0xfu) << 1) | (spread4(bnd[j] >> 8) << 2);
+        }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_merge: one thread per bond slot that crosses a tile face (family k: sites whose coordinate k is
-// the last of its tile; includes the periodic wrap faces).  Lock-free min-root union with retry.
+// Global union-find over the packed label words.  Loads bypass L1 (volatile): other CTAs update
+// parents concurrently.  A root is only ever changed by the atomicCAS that hooks it; path halving
+// rewrites non-roots with (valid) ancestors, keeping their draw field.
+// ------------------------------------------------------------------------------------------------
+template <int LOG2NS, int TX, int TY>
+__device__ __forceinline__ uint32_t linear_of(const Params &p, uint32_t a)
+{
+    const uint32_t li = a & ((1u << LOG2NS) - 1u);
+    return p.tile_origin[a >> LOG2NS] + (li % TX) + p.L * (((li / TX) % TY) + p.L * (li / (TX * TY)));
+}
+
+__device__ __forceinline__ uint32_t find_g(uint32_t *lab, uint32_t x, int db, uint32_t &rootword, unsigned &hops)
+{
+    volatile uint32_t *vl = lab;
+    const uint32_t dm = (1u << db) - 1u;
+    for (;;) {
+        const uint32_t w = vl[x];
+        const uint32_t px = w >> db;
+        if (px == x) { rootword = w; return x; }
+        const uint32_t w2 = vl[px];
+        const uint32_t gp = w2 >> db;
+        ++hops;
+        if (gp == px) { rootword = w2; return px; }
+        vl[x] = (gp << db) | (w & dm);  // path halving
+        x = gp;
+        ++hops;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// k_merge: one thread per face-bond slot of every tile; threads whose bit is clear leave at once.
 // Thread 0 also clears the magnetisation accumulators that k_flip adds to.
 // ------------------------------------------------------------------------------------------------
 template <int DIM, int TX, int TY, int TZ>
 __global__ void __launch_bounds__(256) k_merge(const Params p)
 {
-    const uint32_t L = p.L;
-    const uint32_t n0 = p.N / TX, n1 = p.N / TY, n2 = (DIM == 3) ? p.N / TZ : 0u;
-    uint32_t s = blockIdx.x * 256u + threadIdx.x;
-    if (s == 0) {
+    using G = TileGeom<DIM, TX, TY, TZ>;
+    constexpr uint32_t SPT = 32u * G::NFW;
+    const uint32_t gid = blockIdx.x * 256u + threadIdx.x;
+    if (gid == 0) {
         p.acc->M_int = 0ull; p.acc->mx = 0.0; p.acc->my = 0.0;
         for (int k = 0; k < p.q; ++k) p.acc->nk[k] = 0ull;
     }
-    uint32_t i, j;
-    int k;
-    if (s < n0) {
-        k = 0;
-        const uint32_t ntx = L / TX;
-        const uint32_t xt = s % ntx, rest = s / ntx;
-        const uint32_t x = xt * TX + (TX - 1);
-        i = x + L * rest;
-        j = (x + 1 == L) ? i - (L - 1) : i + 1;
-    } else if (s < n0 + n1) {
-        k = 1;
-        s -= n0;
-        const uint32_t nty = L / TY;
-        const uint32_t x = s % L, rest = s / L;
-        const uint32_t yt = rest % nty, z = rest / nty;
-        const uint32_t y = yt * TY + (TY - 1);
-        i = x + L * (y + L * z);
-        j = (y + 1 == L) ? i - L * (L - 1) : i + L;
-    } else if (s < n0 + n1 + n2) {
-        k = 2;
-        s -= n0 + n1;
-        const uint32_t LL = L * L;
-        const uint32_t xy = s % LL, zt = s / LL;
-        const uint32_t z = zt * TZ + (TZ - 1);
-        i = xy + LL * z;
-        j = (z + 1 == L) ? xy : i + LL;
+    const uint32_t tile = gid / SPT, slot = gid % SPT;
+    if (tile >= p.ntiles) return;
+    const uint32_t fw = p.faces[tile * G::NFW + (slot >> 5)];
+    if (!((fw >> (slot & 31u)) & 1u)) return;
+    const uint32_t tx = tile % p.ntx, rr = tile / p.ntx, ty = rr % p.nty, tz = rr / p.nty;
+    uint32_t li_i, li_j, tile_j;
+    if (slot < 32u * G::FXW) {
+        const uint32_t r = slot;  // r = ly + TY lz
+        li_i = (TX - 1) + TX * r;
+        li_j = TX * r;
+        tile_j = (tx + 1 == p.ntx) ? tile - (p.ntx - 1) : tile + 1;
+    } else if (slot < 32u * (G::FXW + G::FYW)) {
+        const uint32_t b = slot - 32u * G::FXW;  // b = lx + TX lz
+        li_j = (b % TX) + (TX * TY) * (b / TX);
+        li_i = li_j + TX * (TY - 1);
+        tile_j = (ty + 1 == p.nty) ? tile - p.ntx * (p.nty - 1) : tile + p.ntx;
     } else {
-        return;
+        const uint32_t b = slot - 32u * (G::FXW + G::FYW);  // b = lx + TX ly
+        li_j = b;
+        li_i = b + TX * TY * (TZ - 1);
+        tile_j = (tz + 1 == p.ntz) ? tile - p.ntx * p.nty * (p.ntz - 1) : tile + p.ntx * p.nty;
     }
-    const bool active = (p.bonds[i] >> k) & 1u;
-    if (p.counting) {
-        atomicAdd(&p.acc->stats[0], 1ull);
-        if (active) atomicAdd(&p.acc->stats[1], 1ull);
-    }
-    if (!active) return;
-    uint32_t a = p.labels[i], b = p.labels[j];
-    unsigned hops = 0, retries = 0, linked = 0, maxhops = 0;
+    const int db = p.db;
+    const uint32_t dm = (1u << db) - 1u;
+    uint32_t a = (tile << G::LOG2NS) + li_i, b = (tile_j << G::LOG2NS) + li_j;
+    unsigned hops = 0, retries = 0, linked = 0;
     for (;;) {
-        unsigned h = 0;
-        a = find_g(p.labels, a, h);
-        b = find_g(p.labels, b, h);
-        hops += h;
-        maxhops = h > maxhops ? h : maxhops;
+        uint32_t wa, wb;
+        a = find_g(p.labels, a, db, wa, hops);
+        b = find_g(p.labels, b, db, wb, hops);
         if (a == b) break;
-        if (a < b) { const uint32_t t = a; a = b; b = t; }
-        const uint32_t old = atomicMin(&p.labels[a], b);
-        if (old == a) { linked = 1; break; }
-        a = old;
-        ++retries;
+        if (linear_of<G::LOG2NS, TX, TY>(p, a) < linear_of<G::LOG2NS, TX, TY>(p, b)) {
+            const uint32_t t = a; a = b; b = t;
+            wa = wb;
+        }
+        // a is the root with the larger linear index: hook it under b (keeping a's draw field)
+        const uint32_t old = atomicCAS(&p.labels[a], wa, (b << db) | (wa & dm));
+        if (old == wa) { linked = 1; break; }
+        ++retries;  // a was hooked by another thread meanwhile: find again from there
     }
     if (p.counting) {
+        atomicAdd(&p.acc->stats[1], 1ull);
         atomicAdd(&p.acc->stats[2], (unsigned long long)linked);
         atomicAdd(&p.acc->stats[3], (unsigned long long)retries);
         atomicAdd(&p.acc->stats[4], (unsigned long long)hops);
-        atomicMax(&p.acc->stats[5], (unsigned long long)maxhops);
+        atomicMax(&p.acc->stats[5], (unsigned long long)hops);
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_flip: one CTA per tile.
-//   phase A   every site reads its parent; sites whose parent is themselves or lies outside the tile
-//             (the former tile-local roots) are compacted into a list, the others park a tile-local
-//             pointer in smem
-//   phase A2  the list is processed densely, one root per thread: chase the global root r, draw the
-//             cluster's new value from word 3 of Philox(r, t), park (r, draw) in smem
-//   phase B   the other sites follow the tile-local pointers in smem to a parked entry
-//   then      new spin / XY reflection written in place, magnetisation sums reduced per CTA
+// k_flip: one CTA per tile, QPT quads per thread.  Every site follows its parent words to the root
+// (first hop: the tile-local root, whose word sits in this tile's 4*NS-byte block and is served by
+// L1; further hops only for clusters that cross tile faces), takes the root's draw field as the
+// cluster's new value and writes its spin; magnetisation sums per CTA.
 // ------------------------------------------------------------------------------------------------
-constexpr uint32_t LOCAL_PTR = 0x80000000u;
-
 template <int DIM, int MODEL, int TX, int TY, int TZ, int NT>
 __global__ void __launch_bounds__(NT) k_flip(const Params p)
 {
-    using G = TileGeom<DIM, MODEL, TX, TY, TZ>;
-    constexpr int NS = G::NS;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint32_t *res_s = reinterpret_cast<uint32_t *>(smem_raw);
-    uint16_t *root_s = reinterpret_cast<uint16_t *>(smem_raw + (size_t)NS * 4);
-    uint8_t *draw_s = reinterpret_cast<uint8_t *>(smem_raw + (size_t)NS * 6);
+    using G = TileGeom<DIM, TX, TY, TZ>;
+    constexpr int NS = G::NS, NQ = NS / 4, QPT = NQ / NT;
     __shared__ unsigned long long hist_s[256];
-    __shared__ double red_s[2][32];
-    __shared__ int count_s;
+    __shared__ int red_s[32];
 
     const uint32_t L = p.L;
     const uint32_t x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = (DIM == 3) ? blockIdx.z * TZ : 0u;
-    const int tid = threadIdx.x;
-    constexpr int ROWS = NS / 32, NW = NT / 32;
-    const int lane = tid & 31, warp = tid >> 5;
-    const uint32_t below = (1u << lane) - 1u;
+    const uint32_t tile = blockIdx.x + p.ntx * (blockIdx.y + p.nty * blockIdx.z);
+    const uint32_t tile_base = tile << G::LOG2NS;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int db = (MODEL == POTTS) ? p.db : 1;
+    const uint32_t dm = (1u << db) - 1u;
+    const uint32_t *__restrict__ lab = p.labels;
 
-    if (tid == 0) count_s = 0;
     if (MODEL == POTTS) {
         for (int k = tid; k < 256; k += NT) hist_s[k] = 0ull;
+        __syncthreads();
     }
-    __syncthreads();
-
-    for (int row = warp; row < ROWS; row += NW) {
-        const int li = row * 32 + lane;
-        const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
-        const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
-        const uint32_t par = p.labels[g];
-        uint32_t px, py, pz;
-        decode(p, par, px, py, pz);
-        const uint32_t dx = px - x0, dy = py - y0, dz = pz - z0;
-        const bool in_tile = dx < (uint32_t)TX && dy < (uint32_t)TY && dz < (uint32_t)TZ;
-        const bool is_root = (par == g) || !in_tile;
-        res_s[li] = is_root ? par : (LOCAL_PTR | (dx + TX * (dy + TY * dz)));
-        const uint32_t m = __ballot_sync(FULL, is_root);
-        int base = 0;
-        if (lane == 0 && m) base = atomicAdd(&count_s, __popc(m));
-        base = __shfl_sync(FULL, base, 0);
-        if (is_root) root_s[base + __popc(m & below)] = (uint16_t)li;
-    }
-    __syncthreads();
-
-    const int nroots = count_s;
-    unsigned chase_hops = 0, chase_max = 0;
-    for (int e0 = 0; e0 < nroots; e0 += NT) {
-        const int e = e0 + tid;
-        if (e < nroots) {
-            const int li = root_s[e];
-            uint32_t r = res_s[li], n;
-            unsigned h = 0;
-            while ((n = p.labels[r]) != r) { r = n; ++h; }
-            chase_hops += h;
-            chase_max = h > chase_max ? h : chase_max;
-            const uint32_t w = philox4x32_10(r, p.t_lo, p.t_hi, DOM_SITE, p.k0, p.k1).w;
-            res_s[li] = r;
-            draw_s[li] = (MODEL == POTTS) ? (uint8_t)(((unsigned long long)w * (unsigned)p.q) >> 32)
-                                          : (uint8_t)(w >> 31);
+    int m_loc = 0;
+    unsigned chase_hops = 0;
+#pragma unroll
+    for (int j = 0; j < QPT; ++j) {
+        const int li = (tid + j * NT) * 4;
+        const uint32_t a0 = tile_base + li;
+        const uint4 w4 = *reinterpret_cast<const uint4 *>(lab + a0);
+        uint32_t pw[4] = {w4.x, w4.y, w4.z, w4.w};
+        uint32_t tgt[4];
+        bool pend[4], same[4];
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            tgt[s] = pw[s] >> db;
+            same[s] = s > 0 && tgt[s] == tgt[s - 1];
+            pend[s] = tgt[s] != a0 + s && !same[s];
+        }
+        while (pend[0] | pend[1] | pend[2] | pend[3]) {
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                if (pend[s]) {
+                    const uint32_t nw = __ldg(lab + tgt[s]);
+                    const uint32_t np = nw >> db;
+                    ++chase_hops;
+                    if (np == tgt[s]) { pw[s] = nw; pend[s] = false; }
+                    else tgt[s] = np;
+                }
+            }
         }
         __syncwarp();
-    }
-    __syncthreads();
+#pragma unroll
+        for (int s = 1; s < 4; ++s)
+            if (same[s]) pw[s] = pw[s - 1];
 
-    long long m_loc = 0;
-    double cx = 0.0, cy = 0.0;
-    for (int row = warp; row < ROWS; row += NW) {
-        const int li = row * 32 + lane;
         const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
         const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
-        uint32_t at = li, v = res_s[li];
-        while (v & LOCAL_PTR) { at = v & ~LOCAL_PTR; v = res_s[at]; }
-        __syncwarp();
-        const uint32_t d = draw_s[at];
         if (MODEL == ISING) {
             // "All spins in each cluster are set randomly to +1 or -1"
-            const int s = d ? 1 : -1;
-            ((int8_t *)p.spins)[g] = (int8_t)s;
-            m_loc += s;
+            const uint32_t dn = (pw[0] & 1u) | ((pw[1] & 1u) << 1) | ((pw[2] & 1u) << 2) | ((pw[3] & 1u) << 3);
+            *reinterpret_cast<uint32_t *>((uint8_t *)p.spins + g) = 0xffffffffu ^ (spread4(dn) * 0xfeu);
+            m_loc += 2 * __popc(dn) - 4;
         } else if (MODEL == POTTS) {
-            ((uint8_t *)p.spins)[g] = (uint8_t)d;
-            if (p.q <= 8) {
-                for (int k = 0; k < p.q; ++k) {
-                    const unsigned c = __popc(__ballot_sync(FULL, d == (uint32_t)k));
-                    if (lane == 0) atomicAdd(&hist_s[k], (unsigned long long)c);
-                }
-            } else {
-                atomicAdd(&hist_s[d], 1ull);
-            }
+            const uint32_t d0 = pw[0] & dm, d1 = pw[1] & dm, d2 = pw[2] & dm, d3 = pw[3] & dm;
+            *reinterpret_cast<uint32_t *>((uint8_t *)p.spins + g) = d0 | (d1 << 8) | (d2 << 16) | (d3 << 24);
+            atomicAdd(&hist_s[d0], 1ull);
+            atomicAdd(&hist_s[d1], 1ull);
+            atomicAdd(&hist_s[d2], 1ull);
+            atomicAdd(&hist_s[d3], 1ull);
         } else {
             // PAPER.md:159 mirror projection: theta' = c - theta, wrapped into [0, 2 pi]
-            float th = ((float *)p.spins)[g];
-            if (d) {
-                th = p.crefl - th;
-                if (th < 0.0f) th = th + 6.283185307179586476925286766559f;
-                ((float *)p.spins)[g] = th;
+            if ((pw[0] | pw[1] | pw[2] | pw[3]) & 1u) {
+                float4 t4 = *reinterpret_cast<float4 *>((float *)p.spins + g);
+                float th[4] = {t4.x, t4.y, t4.z, t4.w};
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    if (pw[s] & 1u) {
+                        float v = p.crefl - th[s];
+                        if (v < 0.0f) v = v + 6.283185307179586476925286766559f;
+                        th[s] = v;
+                    }
+                }
+                *reinterpret_cast<float4 *>((float *)p.spins + g) = make_float4(th[0], th[1], th[2], th[3]);
             }
-            float sn, cs;
-            sincosf(th, &sn, &cs);
-            cx += (double)cs;
-            cy += (double)sn;
         }
     }
 
     if (MODEL == ISING) {
-        int m = (int)m_loc;
-        m = __reduce_add_sync(FULL, m);
-        if (lane == 0) atomicAdd(&p.acc->M_int, (unsigned long long)(long long)m);
+        m_loc = __reduce_add_sync(FULL, m_loc);
+        if (lane == 0) red_s[warp] = m_loc;
+        __syncthreads();
+        if (warp == 0) {
+            int v = lane < NT / 32 ? red_s[lane] : 0;
+            v = __reduce_add_sync(FULL, v);
+            if (lane == 0) atomicAdd(&p.acc->M_int, (unsigned long long)(long long)v);
+        }
     } else if (MODEL == POTTS) {
         __syncthreads();
         for (int k = tid; k < p.q; k += NT)
             if (hist_s[k]) atomicAdd(&p.acc->nk[k], hist_s[k]);
-    } else {
-        for (int o = 16; o > 0; o >>= 1) {
-            cx += __shfl_down_sync(FULL, cx, o);
-            cy += __shfl_down_sync(FULL, cy, o);
-        }
-        if (lane == 0) { red_s[0][warp] = cx; red_s[1][warp] = cy; }
-        __syncthreads();
-        if (warp == 0) {
-            cx = lane < NW ? red_s[0][lane] : 0.0;
-            cy = lane < NW ? red_s[1][lane] : 0.0;
-            for (int o = 16; o > 0; o >>= 1) {
-                cx += __shfl_down_sync(FULL, cx, o);
-                cy += __shfl_down_sync(FULL, cy, o);
-            }
-            if (lane == 0) { atomicAdd(&p.acc->mx, cx); atomicAdd(&p.acc->my, cy); }
-        }
     }
     if (p.counting) {
         atomicAdd(&p.acc->stats[6], (unsigned long long)chase_hops);
-        atomicMax(&p.acc->stats[7], (unsigned long long)chase_max);
+        atomicMax(&p.acc->stats[7], (unsigned long long)chase_hops);
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_flatten: label[i] <- root of i, in place (parents only decrease, so concurrent readers are safe).
-// Only run on request (sw_get_labels): the step itself never needs the flat array.
+// k_export_labels: canonical labels on request (sw_get_labels): labels_out[i] = minimum linear site
+// index of the cluster of site i, linear order.  Not on the hot path.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_flatten(const Params p)
+template <int DIM, int TX, int TY, int TZ>
+__global__ void __launch_bounds__(256) k_export_labels(const Params p)
 {
+    using G = TileGeom<DIM, TX, TY, TZ>;
     const uint32_t i = blockIdx.x * 256u + threadIdx.x;
     if (i >= p.N) return;
-    uint32_t r = p.labels[i], n;
-    while ((n = p.labels[r]) != r) r = n;
-    p.labels[i] = r;
+    uint32_t x, y, z;
+    decode(p, i, x, y, z);
+    const uint32_t tile = x / TX + p.ntx * (y / TY + p.nty * (z / TZ));
+    uint32_t a = (tile << G::LOG2NS) + (x % TX) + TX * ((y % TY) + TY * (z % TZ));
+    const int db = p.db;
+    for (;;) {
+        const uint32_t n = p.labels[a] >> db;
+        if (n == a) break;
+        a = n;
+    }
+    p.labels_out[i] = linear_of<G::LOG2NS, TX, TY>(p, a);
 }
 
 // ------------------------------------------------------------------------------------------------

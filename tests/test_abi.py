@@ -29,15 +29,17 @@ def test_library_exports_every_declared_symbol():
 def test_workspace_bytes_and_validation_without_device():
     from paper_1403_7560_b200 import binding
     lib = binding.lib()
-    # 3D L=512 Ising: spins N + bonds N + labels 4N + accumulators
+    # 3D L=512 Ising: spins N + bonds N + labels 4N + face words, tile origins, accumulators (< N/8)
     n = 512 ** 3
     b = lib.sw_workspace_bytes(3, 512, binding.ISING, 0)
-    assert 6 * n <= b <= 6 * n + 4096 * 4
+    assert 6 * n <= b <= 6 * n + n // 8
     assert lib.sw_workspace_bytes(3, 256, binding.XY, 0) >= 9 * 256 ** 3
     assert lib.sw_workspace_bytes(2, 48, binding.ISING, 0) == 0      # not a multiple of 32
     assert lib.sw_workspace_bytes(4, 64, binding.ISING, 0) == 0      # dim
     assert lib.sw_workspace_bytes(2, 64, binding.POTTS, 1) == 0      # q
     assert lib.sw_workspace_bytes(3, 2048, binding.ISING, 0) == 0    # N > 2^31
+    assert lib.sw_workspace_bytes(3, 1024, binding.POTTS, 3) > 0     # 2^30 sites x 2 state bits
+    assert lib.sw_workspace_bytes(3, 1024, binding.POTTS, 5) == 0    # 2^30 sites x 3 state bits > 2^32
     h = C.c_void_p()
     rc = lib.sw_create(C.byref(h), 2, 48, binding.ISING, 0, 0.4, 1)
     assert rc == binding.SW_EINVAL and not h

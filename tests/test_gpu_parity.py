@@ -64,7 +64,7 @@ def test_philox_device_known_answers():
 ])
 def test_full_trajectory_bit_exact(dim, L, model, q, T, steps):
     sw, orc = _mods()
-    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=1)
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=1, record_bonds=True)
     o = orc.Oracle(dim, L, model, q, 1.0 / T, 1)
     assert np.array_equal(g.spins(), o.spins()), "seeded start differs"
     assert g.counts() == o.counts()
@@ -77,11 +77,11 @@ def test_full_trajectory_bit_exact(dim, L, model, q, T, steps):
     assert (e, m, m2, m4) == pytest.approx(o.observables(), rel=1e-14)
 
 
-@pytest.mark.parametrize("tile", ["32x32", "64x32", "128x16", "128x32"])
+@pytest.mark.parametrize("tile", ["32x32", "64x64", "128x32", "128x64"])
 def test_tile_menu_2d(tile, monkeypatch):
     sw, orc = _mods()
     monkeypatch.setenv("SW_B200_TILE", tile)
-    g = sw.SwendsenWang(2, 256, 0, 0, 1.0 / TC2, seed=5)
+    g = sw.SwendsenWang(2, 256, 0, 0, 1.0 / TC2, seed=5, record_bonds=True)
     o = orc.Oracle(2, 256, 0, 0, 1.0 / TC2, 5)
     for t in range(25):
         g.step(1)
@@ -93,7 +93,7 @@ def test_tile_menu_2d(tile, monkeypatch):
 def test_tile_menu_3d(tile, monkeypatch):
     sw, orc = _mods()
     monkeypatch.setenv("SW_B200_TILE", tile)
-    g = sw.SwendsenWang(3, 64, 0, 0, 1.0 / T3, seed=5)
+    g = sw.SwendsenWang(3, 64, 0, 0, 1.0 / T3, seed=5, record_bonds=True)
     o = orc.Oracle(3, 64, 0, 0, 1.0 / T3, 5)
     for t in range(12):
         g.step(1)
@@ -107,14 +107,14 @@ def test_edge_beta_zero_and_cold_start(dim, L, model, q):
     sw, orc = _mods()
     from paper_1403_7560_b200 import inputs
     N = L ** dim
-    g = sw.SwendsenWang(dim, L, model, q, 0.0, seed=3)
+    g = sw.SwendsenWang(dim, L, model, q, 0.0, seed=3, record_bonds=True)
     o = orc.Oracle(dim, L, model, q, 0.0, 3)
     g.step(1)
     o.step(1)
     assert not g.bonds().any()
     assert np.array_equal(g.labels(), np.arange(N, dtype=np.uint32))
     _compare_step(g, o, "beta=0")
-    g = sw.SwendsenWang(dim, L, model, q, 40.0, seed=3)
+    g = sw.SwendsenWang(dim, L, model, q, 40.0, seed=3, record_bonds=True)
     o = orc.Oracle(dim, L, model, q, 40.0, 3)
     cold = inputs.aligned_spins(model, N)
     g.set_spins(cold, 7)
@@ -132,7 +132,7 @@ def test_injected_structured_states(dim, L, model, q, T):
     """Stripes and block domains at low T: long clusters crossing many tiles and the wrap faces."""
     sw, orc = _mods()
     from paper_1403_7560_b200 import inputs
-    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=11)
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=11, record_bonds=True)
     o = orc.Oracle(dim, L, model, q, 1.0 / T, 11)
     states = [inputs.striped_spins(model, dim, L, 5, max(q, 2)),
               inputs.domain_spins(model, dim, L, 24, max(q, 2), seed=2),
@@ -149,7 +149,7 @@ def test_injected_structured_states(dim, L, model, q, T):
 def test_labels_are_components_independent_check():
     """I2/I3 with scipy's connected_components (neither the oracle's BFS nor the GPU's union-find)."""
     sw, _ = _mods()
-    g = sw.SwendsenWang(3, 64, 0, 0, 1.0 / T3, seed=2)
+    g = sw.SwendsenWang(3, 64, 0, 0, 1.0 / T3, seed=2, record_bonds=True)
     g.step(30)
     before = g.spins()
     g.step(1)
@@ -184,8 +184,8 @@ def test_ising_equals_potts_q2():
     """R1: Ising(beta) == Potts(q=2, 2 beta) bit for bit under s = 2k - 1."""
     sw, _ = _mods()
     beta = 1.0 / TC2
-    a = sw.SwendsenWang(2, 128, 0, 0, beta, seed=4)
-    b = sw.SwendsenWang(2, 128, 1, 2, 2.0 * beta, seed=4)
+    a = sw.SwendsenWang(2, 128, 0, 0, beta, seed=4, record_bonds=True)
+    b = sw.SwendsenWang(2, 128, 1, 2, 2.0 * beta, seed=4, record_bonds=True)
     for t in range(20):
         a.step(1)
         b.step(1)
@@ -196,7 +196,7 @@ def test_ising_equals_potts_q2():
 
 def test_state_errors():
     sw, _ = _mods()
-    g = sw.SwendsenWang(2, 64, 0, 0, 0.4, seed=1)
+    g = sw.SwendsenWang(2, 64, 0, 0, 0.4, seed=1, record_bonds=True)
     with pytest.raises(sw.SwError) as ei:
         g.bonds()
     assert ei.value.code == -4
