@@ -72,6 +72,10 @@ bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
 
 bool pick_ops_model(int model, int dim, int tx, int ty, int tz, TileOps &o)
 {
+#ifdef SW_MENU_MIN  // developer builds: one model, one tile per dimension (fast to compile)
+    if (dim == 3) o = make_ops<3, ISING, 32, 16, 16>(); else o = make_ops<2, ISING, 128, 64, 1>();
+    return model == SW_ISING && tx == o.tx && ty == o.ty && tz == o.tz;
+#endif
     if (model == SW_ISING) return pick_ops<ISING>(dim, tx, ty, tz, o);
     if (model == SW_POTTS) return pick_ops<POTTS>(dim, tx, ty, tz, o);
     return pick_ops<XY>(dim, tx, ty, tz, o);
@@ -115,7 +119,7 @@ bool valid_args(int dim, int L, int model, int q, double beta, bool check_beta)
     return true;
 }
 
-struct Layout { size_t spins, bonds, labels, faces, origin, acc, total; };
+struct Layout { size_t spins, bonds, labels, pairs, origin, acc, total; };
 
 Layout layout(int dim, int L, int model)
 {
@@ -126,8 +130,10 @@ Layout layout(int dim, int L, int model)
     l.spins = off; off += align256(N * (model == SW_XY ? 4 : 1));
     l.bonds = off; off += align256(N);
     l.labels = off; off += align256(N * 4);
-    // face words and tile origins: sized for the smallest tile of the menu (1024 sites, <= 18 words)
-    l.faces = off; off += align256((N / 1024) * 18 * 4);
+    // pair list: one (i, j) address pair per bond through a tile face, sized for the tile of the menu
+    // with the largest face area (3D 32x8x8: (1/32 + 1/8 + 1/8) N bonds; 2D 32x32: N/16); then the
+    // tile origins (smallest tile: 1024 sites)
+    l.pairs = off; off += align256((dim == 3 ? N / 32 * 9 : N / 16) * 8);
     l.origin = off; off += align256((N / 1024) * 4);
     l.acc = off; off += align256(sizeof(Acc));
     l.total = off;
@@ -146,6 +152,7 @@ struct sw_ctx {
     cudaStream_t stream;
     void *workspace;
     uint8_t *bonds_mem;
+    unsigned merge_blocks;
     bool own_workspace, own_stream;
     bool stepped;      // labels of a step are available
     bool bonds_valid;  // the last step recorded its bond bytes
@@ -289,7 +296,8 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     p.bonds = nullptr;
     c->bonds_mem = (uint8_t *)(base + lay.bonds);
     p.labels = (uint32_t *)(base + lay.labels);
-    p.faces = (uint32_t *)(base + lay.faces);
+    p.pairs = (uint2 *)(base + lay.pairs);
+    p.npairs = &((Acc *)(base + lay.acc))->npairs;
     p.tile_origin = (uint32_t *)(base + lay.origin);
     p.labels_out = nullptr;
     p.acc = (Acc *)(base + lay.acc);
@@ -297,6 +305,15 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     p.ntz = (dim == 3) ? (uint32_t)(L / c->ops.tz) : 1u;
     p.ntiles = p.ntx * p.nty * p.ntz;
     p.db = draw_bits(model, q);
+    {   // k_merge: a resident grid that strides over the pair list
+        int dev = 0, sms = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const size_t max_pairs = c->N / c->ops.tx + c->N / c->ops.ty + (dim == 3 ? c->N / c->ops.tz : 0);
+        size_t blocks = (max_pairs + 255) / 256;
+        if (blocks > (size_t)sms * 8) blocks = (size_t)sms * 8;
+        c->merge_blocks = (unsigned)blocks;
+    }
     p.L = (uint32_t)L; p.N = (uint32_t)c->N;
     p.k0 = (uint32_t)(seed & 0xffffffffu); p.k1 = (uint32_t)(seed >> 32);
     p.t_lo = p.t_hi = 0;
@@ -365,7 +382,6 @@ int sw_step(sw_ctx *c, int n)
     if (rc) return rc;
     if (n < 0) return fail(SW_EINVAL, "n < 0");
     const dim3 grid = tile_grid(c);
-    const uint32_t slots = c->p.ntiles * 32u * (uint32_t)c->ops.nfw;
     for (int s = 0; s < n; ++s) {
         Params &p = c->p;
         p.bonds = c->record_bonds ? c->bonds_mem : nullptr;
@@ -391,7 +407,7 @@ int sw_step(sw_ctx *c, int n)
         if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[0], c->stream));
         c->ops.bond_label<<<grid, c->ops.nt, c->ops.smem_bond_label, c->stream>>>(p);
         if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[1], c->stream));
-        c->ops.merge<<<(slots + 255) / 256, 256, 0, c->stream>>>(p);
+        c->ops.merge<<<c->merge_blocks, 256, 0, c->stream>>>(p);
         if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[2], c->stream));
         c->ops.flip<<<grid, c->ops.nt, 0, c->stream>>>(p);
         if (c->timing) {

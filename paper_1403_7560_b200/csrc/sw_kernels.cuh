@@ -29,7 +29,13 @@ enum { ISING = 0, POTTS = 1, XY = 2 };
 constexpr uint32_t DOM_SITE = 0u, DOM_INIT = 2u, DOM_XYDIR = 3u;
 constexpr uint32_t FULL = 0xffffffffu;
 #ifndef SW_BL_THREADS_PER_SM
-#define SW_BL_THREADS_PER_SM 1024  // resident threads per SM k_bond_label is compiled for (register cap)
+#define SW_BL_THREADS_PER_SM 1536  // resident threads per SM k_bond_label is compiled for (register cap)
+#endif
+#ifndef SW_BL_INTERLEAVE
+#define SW_BL_INTERLEAVE 1
+#endif
+#ifndef SW_BL_ROUNDS
+#define SW_BL_ROUNDS 1  // uniform hook + flatten rounds before the general union-find loop
 #endif
 #ifndef SW_BL_JUMPS
 #define SW_BL_JUMPS 2  // pointer-jumping rounds over the tile-local forest before it is stored
@@ -43,13 +49,15 @@ struct Acc {
     double mx, my;               // XY: sum cos, sum sin
     unsigned long long nk[256];  // Potts: n_k
     unsigned long long stats[8]; // see sw_get_label_stats
+    uint32_t npairs;             // length of the pair list of the current step
 };
 
 struct Params {
     void *spins;            // int8 (Ising) | uint8 (Potts) | float (XY angle), N elements, linear order
     uint8_t *bonds;         // N bytes, bit k = bond i -> i + e_k, linear order; NULL = not recorded
     uint32_t *labels;       // N packed parent words, tile-major (see above)
-    uint32_t *faces;        // per tile NFW words: active bonds through the +x, +y, +z tile faces
+    uint2 *pairs;           // compact list of the active bonds through tile faces: (address i, address j)
+    uint32_t *npairs;       // its length (reset by k_flip for the next step)
     uint32_t *tile_origin;  // per tile: linear index of its first site
     uint32_t *labels_out;   // k_export_labels: N canonical labels (minimum linear index), linear order
     Acc *acc;
@@ -108,9 +116,14 @@ struct TileGeom {
     static constexpr int NFW = FXW + FYW + FZW;
     static constexpr int NFWP = (NFW + 3) / 4 * 4;  // padded: what follows in smem stays 16-byte aligned
     static constexpr int NHALO = FXB + FYB + FZB;  // XY: projections of the three plus-faces
+    // smem of k_bond_label (32-bit words): labels, face bit words, their popcount prefix (+ list base,
+    // + leftover count), the list of leftover unions (16-bit entries), XY projections
+    static constexpr int LEFT_CAP = NS / 4;
+    static constexpr int OFF_FACE = NS, OFF_FPRE = NS + NFWP, OFF_LEFT = NS + 2 * NFWP + 4;
+    static constexpr int OFF_VAL = OFF_LEFT + LEFT_CAP / 2;
     template <int MODEL> static constexpr size_t smem_bond_label()
     {
-        return (size_t)NS * 4 + (size_t)NFWP * 4 + (MODEL == XY ? ((size_t)NS + NHALO) * 4 : 0);
+        return (size_t)OFF_VAL * 4 + (MODEL == XY ? ((size_t)NS + NHALO) * 4 : 0);
     }
 };
 
@@ -146,8 +159,19 @@ __device__ __forceinline__ uint32_t find_s(volatile uint32_t *lab, uint32_t x)
 __device__ __forceinline__ void union_s(uint32_t *lab, uint32_t a, uint32_t b)
 {
     for (;;) {
+#if SW_BL_INTERLEAVE
+        {   // both chains in one loop: trip count max(hops a, hops b) instead of the sum, two loads in flight
+            volatile uint32_t *vl = lab;
+            uint32_t pa = vl[a], pb = vl[b];
+            while (pa != a || pb != b) {
+                a = pa; b = pb;
+                pa = vl[a]; pb = vl[b];
+            }
+        }
+#else
         a = find_s(lab, a);
         b = find_s(lab, b);
+#endif
         if (a == b) return;
         if (a < b) { const uint32_t t = a; a = b; b = t; }
         const uint32_t old = atomicMin(&lab[a], b);
@@ -198,18 +222,24 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     static_assert(NQ % NT == 0 && NT % 32 == 0, "whole quads per thread, whole rows per warp");
     static_assert(QPT * WB <= 32, "the work mask of a thread is one 32-bit word");
     extern __shared__ __align__(16) uint32_t smem_u32[];
+    static_assert(G::NFW <= 64, "two face words per lane of warp 0");
+    static_assert(NS <= 32768, "a leftover entry keeps the site in 15 bits");
     uint32_t *lab_s = smem_u32;
-    uint32_t *face_s = smem_u32 + NS;
-    float *val_s = reinterpret_cast<float *>(smem_u32 + NS + G::NFWP);  // XY only: NS + NHALO floats
+    uint32_t *face_s = smem_u32 + G::OFF_FACE;
+    uint32_t *fpre_s = smem_u32 + G::OFF_FPRE;  // NFW prefix counts, [NFWP] = base in the global list, [NFWP+1] = #leftovers, [NFWP+2] = valid part of their list
+    uint16_t *left_s = reinterpret_cast<uint16_t *>(smem_u32 + G::OFF_LEFT);
+    float *val_s = reinterpret_cast<float *>(smem_u32 + G::OFF_VAL);  // XY only: NS + NHALO floats
 
     const uint32_t L = p.L;
-    const uint32_t x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = (DIM == 3) ? blockIdx.z * TZ : 0u;
-    const uint32_t tile = blockIdx.x + p.ntx * (blockIdx.y + p.nty * blockIdx.z);
+    const uint32_t bx = blockIdx.x, by = blockIdx.y, bz = (DIM == 3) ? blockIdx.z : 0u;
+    const uint32_t x0 = bx * TX, y0 = by * TY, z0 = bz * TZ;
+    const uint32_t tile = bx + p.ntx * (by + p.nty * bz);
     const uint32_t tile_base = tile << G::LOG2NS;
     const int tid = threadIdx.x, lane = tid & 31;
     const uint32_t LL = L * L;
 
     if (tid < G::NFW) face_s[tid] = 0u;
+    if (tid == 0) { fpre_s[G::NFWP + 1] = 0u; fpre_s[G::NFWP + 2] = (uint32_t)G::LEFT_CAP; }
 
     if (MODEL == XY) {
         // a_i = r . s_i: interior, then the +x, +y, +z faces (periodic wrap)
@@ -356,6 +386,106 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     }
     __syncthreads();
 
+    if (tid < 32) {
+        // face words are final: exclusive prefix of their popcounts, and room in the global pair list
+        const uint32_t c0 = lane < G::NFW ? __popc(face_s[lane]) : 0u;
+        const uint32_t c1 = lane + 32 < G::NFW ? __popc(face_s[lane + 32]) : 0u;
+        uint32_t i0 = c0, i1 = c1;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u0 = __shfl_up_sync(FULL, i0, o), u1 = __shfl_up_sync(FULL, i1, o);
+            if (lane >= o) { i0 += u0; i1 += u1; }
+        }
+        const uint32_t t0 = __shfl_sync(FULL, i0, 31), t1 = __shfl_sync(FULL, i1, 31);
+        if (lane < G::NFW) fpre_s[lane] = i0 - c0;
+        if (lane + 32 < G::NFW) fpre_s[lane + 32] = t0 + i1 - c1;
+        if (lane == 0) fpre_s[G::NFWP] = (t0 + t1) ? atomicAdd(p.npairs, t0 + t1) : 0u;
+    }
+
+    // phase 2a: SW_BL_ROUNDS uniform hook rounds.  Every thread looks at its quads' bonds with two
+    // 16-byte loads (parents of its 4 sites and of their 4 neighbours); a bond whose two parents differ
+    // tries to hook the larger one under the smaller with a compare-and-swap (parent slot: itself ->
+    // smaller): that succeeds only if the larger one still is a root, and a failure changes nothing
+    // (the bond stays in the work mask).  Straight-line predicated code: no loops, no divergence.
+    // Each round ends with a pointer-jumping pass that re-flattens the forest.
+    const uint32_t lab_sa = (uint32_t)__cvta_generic_to_shared(lab_s);
+#pragma unroll 1
+    for (int round = 0; round < SW_BL_ROUNDS; ++round) {
+#pragma unroll
+        for (int j = 0; j < QPT; ++j) {
+            const int li = (tid + j * NT) * 4;
+            const uint4 la = *reinterpret_cast<const uint4 *>(lab_s + li);
+            const uint32_t av[4] = {la.x, la.y, la.z, la.w};
+#pragma unroll
+            for (int dir = 0; dir < (DIM == 3 ? 2 : 1); ++dir) {
+                const uint32_t nib = (work >> (j * WB + 4 * dir)) & 0xfu;
+                const uint4 lb = *reinterpret_cast<const uint4 *>(lab_s + ((li + (dir ? TX * TY : TX)) & (NS - 1)));
+                const uint32_t bv[4] = {lb.x, lb.y, lb.z, lb.w};
+                uint32_t left = 0u;
+#pragma unroll
+                for (int sidx = 0; sidx < 4; ++sidx) {
+                    const uint32_t hi = max(av[sidx], bv[sidx]), lo = min(av[sidx], bv[sidx]);
+                    const uint32_t need = ((nib >> sidx) & 1u) & (uint32_t)(hi != lo);
+                    uint32_t old = hi;
+                    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
+                                 "@p atom.shared.cas.b32 %0, [%1], %2, %3;\n\t}"
+                                 : "+r"(old) : "r"(lab_sa + 4u * hi), "r"(hi), "r"(lo), "r"(need) : "memory");
+                    left |= (uint32_t)(old != hi) << sidx;
+                }
+                work = (work & ~(0xfu << (j * WB + 4 * dir))) | (left << (j * WB + 4 * dir));
+            }
+        }
+        __syncthreads();
+        volatile uint32_t *vl = lab_s;
+#pragma unroll
+        for (int j = 0; j < QPT; ++j) {
+            const int li = (tid + j * NT) * 4;
+            uint4 r = *reinterpret_cast<const uint4 *>(lab_s + li);
+            r.x = vl[r.x]; r.y = vl[r.y]; r.z = vl[r.z]; r.w = vl[r.w];
+            r.x = vl[r.x]; r.y = vl[r.y]; r.z = vl[r.z]; r.w = vl[r.w];
+            *reinterpret_cast<uint4 *>(lab_s + li) = r;
+        }
+        __syncthreads();
+    }
+    // phase 2b: whatever is left (roots that several bonds wanted to hook at once, deep trees) goes
+    // through the general union-find.  The leftovers of all threads are first compacted into one list
+    // so that every lane of every warp has a union to do (a warp whose entries do not fit keeps them).
+    if (SW_BL_ROUNDS > 0) {
+        const uint32_t cnt = __popc(work);
+        uint32_t inc = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(FULL, inc, o);
+            if (lane >= o) inc += u;
+        }
+        const uint32_t tot = __shfl_sync(FULL, inc, 31);
+        uint32_t base = 0u;
+        if (lane == 31 && tot) base = atomicAdd(&fpre_s[G::NFWP + 1], tot);
+        base = __shfl_sync(FULL, base, 31);
+        if (tot && base + tot <= (uint32_t)G::LEFT_CAP) {
+            uint32_t pos = base + inc - cnt;
+            while (work) {
+                const int k = __ffs(work) - 1;
+                work &= work - 1u;
+                const int jq = k / WB, r = k % WB;
+                left_s[pos++] = (uint16_t)(((tid + jq * NT) * 4 + (r & 3)) | ((r & 4) << 13));
+            }
+        } else if (tot && lane == 31) {
+            atomicMin(&fpre_s[G::NFWP + 2], base);  // the list is valid below the first range that did not fit
+        }
+        __syncthreads();
+        const int nleft = min(fpre_s[G::NFWP + 1], fpre_s[G::NFWP + 2]);
+        // warps whose entries did not fit still hold their bits and run the loop below
+        for (int e0 = (tid & ~31); e0 < nleft; e0 += NT) {
+            const int e = e0 + lane;
+            if (e < nleft) {
+                const uint32_t v = left_s[e];
+                const uint32_t a = v & 0x7fffu;
+                union_s(lab_s, a, a + ((v & 0x8000u) ? (uint32_t)(TX * TY) : (uint32_t)TX));
+            }
+            __syncwarp();
+        }
+    }
     // warp-uniform trip count + __syncwarp: lanes whose union ends early wait for the others instead
     // of drifting into later iterations on their own (that would serialise the warp)
     while (__any_sync(FULL, work != 0u)) {
@@ -370,7 +500,30 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     }
     __syncthreads();
 
-    if (tid < G::NFW) p.faces[tile * G::NFW + tid] = face_s[tid];
+    // active face bonds -> (address of i, address of j) in the global pair list (k_merge's work)
+    {
+        const uint32_t ntx = p.ntx, nty = p.nty;
+        const uint32_t tjx = (bx + 1 == ntx) ? tile - (ntx - 1) : tile + 1;
+        const uint32_t tjy = (by + 1 == nty) ? tile - ntx * (nty - 1) : tile + ntx;
+        const uint32_t tjz = (DIM == 3) ? ((bz + 1 == p.ntz) ? tile - ntx * nty * (p.ntz - 1) : tile + ntx * nty) : 0u;
+        const uint32_t fbase = fpre_s[G::NFWP];
+        for (int sl = tid; sl < 32 * G::NFW; sl += NT) {
+            const uint32_t fw = face_s[sl >> 5];
+            if ((fw >> (sl & 31)) & 1u) {
+                const uint32_t pos = fbase + fpre_s[sl >> 5] + __popc(fw & ((1u << (sl & 31)) - 1u));
+                uint32_t li_i, li_j, tj;
+                if (sl < 32 * G::FXW) {                      // slot = ly + TY lz
+                    li_j = TX * sl; li_i = li_j + (TX - 1); tj = tjx;
+                } else if (sl < 32 * (G::FXW + G::FYW)) {    // slot = lx + TX lz
+                    const uint32_t b = sl - 32 * G::FXW;
+                    li_j = (b % TX) + (TX * TY) * (b / TX); li_i = li_j + TX * (TY - 1); tj = tjy;
+                } else {                                     // slot = lx + TX ly
+                    li_j = sl - 32 * (G::FXW + G::FYW); li_i = li_j + TX * TY * (TZ - 1); tj = tjz;
+                }
+                p.pairs[pos] = make_uint2(tile_base + li_i, (tj << G::LOG2NS) + li_j);
+            }
+        }
+    }
     // phase 3: no unions any more, the forest is static.  JUMPS rounds of pointer jumping (uniform
     // work, no divergence; a thread only rewrites the entries of its own sites, and whatever another
     // thread reads is a valid ancestor), then the parent is stored as it stands: k_merge and k_flip
@@ -413,84 +566,68 @@ __device__ __forceinline__ uint32_t linear_of(const Params &p, uint32_t a)
     return p.tile_origin[a >> LOG2NS] + (li % TX) + p.L * (((li / TX) % TY) + p.L * (li / (TX * TY)));
 }
 
-__device__ __forceinline__ uint32_t find_g(uint32_t *lab, uint32_t x, int db, uint32_t &rootword, unsigned &hops)
-{
-    volatile uint32_t *vl = lab;
-    const uint32_t dm = (1u << db) - 1u;
-    for (;;) {
-        const uint32_t w = vl[x];
-        const uint32_t px = w >> db;
-        if (px == x) { rootword = w; return x; }
-        const uint32_t w2 = vl[px];
-        const uint32_t gp = w2 >> db;
-        ++hops;
-        if (gp == px) { rootword = w2; return px; }
-        vl[x] = (gp << db) | (w & dm);  // path halving
-        x = gp;
-        ++hops;
-    }
-}
-
 // ------------------------------------------------------------------------------------------------
-// k_merge: one thread per face-bond slot of every tile; threads whose bit is clear leave at once.
-// Thread 0 also clears the magnetisation accumulators that k_flip adds to.
+// k_merge: grid-stride loop over the compact pair list.  Union of (a, b): both chains are followed in
+// one loop (two loads in flight), path splitting on the way (non-roots are re-pointed to their
+// grandparent with plain stores, keeping their draw field); then the root with the larger linear
+// index is hooked under the other with atomicCAS(root word -> parent word); a lost race starts
+// over from the roots found.  Thread 0 also clears the magnetisation accumulators k_flip adds to.
 // ------------------------------------------------------------------------------------------------
 template <int DIM, int TX, int TY, int TZ>
 __global__ void __launch_bounds__(256) k_merge(const Params p)
 {
     using G = TileGeom<DIM, TX, TY, TZ>;
-    constexpr uint32_t SPT = 32u * G::NFW;
     const uint32_t gid = blockIdx.x * 256u + threadIdx.x;
     if (gid == 0) {
         p.acc->M_int = 0ull; p.acc->mx = 0.0; p.acc->my = 0.0;
         for (int k = 0; k < p.q; ++k) p.acc->nk[k] = 0ull;
     }
-    const uint32_t tile = gid / SPT, slot = gid % SPT;
-    if (tile >= p.ntiles) return;
-    const uint32_t fw = p.faces[tile * G::NFW + (slot >> 5)];
-    if (!((fw >> (slot & 31u)) & 1u)) return;
-    const uint32_t tx = tile % p.ntx, rr = tile / p.ntx, ty = rr % p.nty, tz = rr / p.nty;
-    uint32_t li_i, li_j, tile_j;
-    if (slot < 32u * G::FXW) {
-        const uint32_t r = slot;  // r = ly + TY lz
-        li_i = (TX - 1) + TX * r;
-        li_j = TX * r;
-        tile_j = (tx + 1 == p.ntx) ? tile - (p.ntx - 1) : tile + 1;
-    } else if (slot < 32u * (G::FXW + G::FYW)) {
-        const uint32_t b = slot - 32u * G::FXW;  // b = lx + TX lz
-        li_j = (b % TX) + (TX * TY) * (b / TX);
-        li_i = li_j + TX * (TY - 1);
-        tile_j = (ty + 1 == p.nty) ? tile - p.ntx * (p.nty - 1) : tile + p.ntx;
-    } else {
-        const uint32_t b = slot - 32u * (G::FXW + G::FYW);  // b = lx + TX ly
-        li_j = b;
-        li_i = b + TX * TY * (TZ - 1);
-        tile_j = (tz + 1 == p.ntz) ? tile - p.ntx * p.nty * (p.ntz - 1) : tile + p.ntx * p.nty;
-    }
+    const uint32_t n = *p.npairs;
     const int db = p.db;
     const uint32_t dm = (1u << db) - 1u;
-    uint32_t a = (tile << G::LOG2NS) + li_i, b = (tile_j << G::LOG2NS) + li_j;
-    unsigned hops = 0, retries = 0, linked = 0;
-    for (;;) {
-        uint32_t wa, wb;
-        a = find_g(p.labels, a, db, wa, hops);
-        b = find_g(p.labels, b, db, wb, hops);
-        if (a == b) break;
-        if (linear_of<G::LOG2NS, TX, TY>(p, a) < linear_of<G::LOG2NS, TX, TY>(p, b)) {
-            const uint32_t t = a; a = b; b = t;
-            wa = wb;
+    volatile uint32_t *vl = p.labels;
+    for (uint32_t i = gid; i < n; i += gridDim.x * 256u) {
+        const uint2 ab = p.pairs[i];
+        uint32_t a = ab.x, b = ab.y;
+        unsigned hops = 0, retries = 0, linked = 0;
+        uint32_t wa = vl[a], wb = vl[b];
+        for (;;) {
+            for (;;) {
+                const uint32_t pa = wa >> db, pb = wb >> db;
+                const bool ra = pa == a, rb = pb == b;
+                if (ra && rb) break;
+                uint32_t wpa = 0u, wpb = 0u;
+                if (!ra) wpa = vl[pa];
+                if (!rb) wpb = vl[pb];
+                if (!ra) {
+                    const uint32_t gp = wpa >> db;
+                    if (gp != pa) vl[a] = (gp << db) | (wa & dm);
+                    a = pa; wa = wpa; ++hops;
+                }
+                if (!rb) {
+                    const uint32_t gp = wpb >> db;
+                    if (gp != pb) vl[b] = (gp << db) | (wb & dm);
+                    b = pb; wb = wpb; ++hops;
+                }
+            }
+            if (a == b) break;
+            if (linear_of<G::LOG2NS, TX, TY>(p, a) < linear_of<G::LOG2NS, TX, TY>(p, b)) {
+                const uint32_t t = a; a = b; b = t;
+                const uint32_t tw = wa; wa = wb; wb = tw;
+            }
+            // a is the root with the larger linear index: hook it under b (keeping a's draw field)
+            const uint32_t old = atomicCAS(&p.labels[a], wa, (b << db) | (wa & dm));
+            if (old == wa) { linked = 1; break; }
+            wa = old;  // a was hooked by another thread meanwhile: go on from its new word
+            ++retries;
         }
-        // a is the root with the larger linear index: hook it under b (keeping a's draw field)
-        const uint32_t old = atomicCAS(&p.labels[a], wa, (b << db) | (wa & dm));
-        if (old == wa) { linked = 1; break; }
-        ++retries;  // a was hooked by another thread meanwhile: find again from there
-    }
-    if (p.counting) {
-        atomicAdd(&p.acc->stats[1], 1ull);
-        atomicAdd(&p.acc->stats[2], (unsigned long long)linked);
-        atomicAdd(&p.acc->stats[3], (unsigned long long)retries);
-        atomicAdd(&p.acc->stats[4], (unsigned long long)hops);
-        atomicMax(&p.acc->stats[5], (unsigned long long)hops);
+        if (p.counting) {
+            atomicAdd(&p.acc->stats[1], 1ull);
+            atomicAdd(&p.acc->stats[2], (unsigned long long)linked);
+            atomicAdd(&p.acc->stats[3], (unsigned long long)retries);
+            atomicAdd(&p.acc->stats[4], (unsigned long long)hops);
+            atomicMax(&p.acc->stats[5], (unsigned long long)hops);
+        }
     }
 }
 
@@ -505,7 +642,7 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
 {
     using G = TileGeom<DIM, TX, TY, TZ>;
     constexpr int NS = G::NS, NQ = NS / 4, QPT = NQ / NT;
-    __shared__ unsigned long long hist_s[256];
+    __shared__ uint32_t hist_s[256];  // Potts: n_k of this tile (<= NS, fits 32 bits)
     __shared__ int red_s[32];
 
     const uint32_t L = p.L;
@@ -518,10 +655,12 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
     const uint32_t *__restrict__ lab = p.labels;
 
     if (MODEL == POTTS) {
-        for (int k = tid; k < 256; k += NT) hist_s[k] = 0ull;
+        for (int k = tid; k < 256; k += NT) hist_s[k] = 0u;
         __syncthreads();
     }
+    if (tile == 0 && tid == 0) *p.npairs = 0u;  // k_merge of this step is done: empty list for the next one
     int m_loc = 0;
+    uint32_t cnt_lo = 0u, cnt_hi = 0u;  // Potts, q <= 8: per-thread counts of states 0-3 / 4-7, one byte each
     unsigned chase_hops = 0;
 #pragma unroll
     for (int j = 0; j < QPT; ++j) {
@@ -564,10 +703,19 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
         } else if (MODEL == POTTS) {
             const uint32_t d0 = pw[0] & dm, d1 = pw[1] & dm, d2 = pw[2] & dm, d3 = pw[3] & dm;
             *reinterpret_cast<uint32_t *>((uint8_t *)p.spins + g) = d0 | (d1 << 8) | (d2 << 16) | (d3 << 24);
-            atomicAdd(&hist_s[d0], 1ull);
-            atomicAdd(&hist_s[d1], 1ull);
-            atomicAdd(&hist_s[d2], 1ull);
-            atomicAdd(&hist_s[d3], 1ull);
+            if (p.q <= 8) {
+                const uint32_t dv[4] = {d0, d1, d2, d3};
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    const uint32_t inc = 1u << ((dv[s] & 3u) * 8u);
+                    if (dv[s] & 4u) cnt_hi += inc; else cnt_lo += inc;
+                }
+            } else {
+                atomicAdd(&hist_s[d0], 1u);
+                atomicAdd(&hist_s[d1], 1u);
+                atomicAdd(&hist_s[d2], 1u);
+                atomicAdd(&hist_s[d3], 1u);
+            }
         } else {
             // PAPER.md:159 mirror projection: theta' = c - theta, wrapped into [0, 2 pi]
             if ((pw[0] | pw[1] | pw[2] | pw[3]) & 1u) {
@@ -596,9 +744,17 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
             if (lane == 0) atomicAdd(&p.acc->M_int, (unsigned long long)(long long)v);
         }
     } else if (MODEL == POTTS) {
+        if (p.q <= 8) {
+            // a thread counted at most 4 QPT <= 255 sites per state: bytes cannot overflow
+            for (int k = 0; k < p.q; ++k) {
+                const uint32_t c = ((k < 4 ? cnt_lo : cnt_hi) >> ((k & 3) * 8)) & 0xffu;
+                const uint32_t w = __reduce_add_sync(FULL, c);
+                if (lane == 0 && w) atomicAdd(&hist_s[k], w);
+            }
+        }
         __syncthreads();
         for (int k = tid; k < p.q; k += NT)
-            if (hist_s[k]) atomicAdd(&p.acc->nk[k], hist_s[k]);
+            if (hist_s[k]) atomicAdd(&p.acc->nk[k], (unsigned long long)hist_s[k]);
     }
     if (p.counting) {
         atomicAdd(&p.acc->stats[6], (unsigned long long)chase_hops);
