@@ -40,11 +40,15 @@ void swo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* Reading S2: key = (seed low, seed high); counter = (site, t low, t high, domain).
- * Domain SITE: one call per site and step; word k (k < dim) decides the bond in direction k,
- * word 3 is the new value of the cluster whose root (minimum site index) is this site.
+/* Reading 6: key = (seed low, seed high); counter = (index, t low, t high, domain).
+ * Domain SITE (Potts, XY): one call per site and step, index = site; word k (k < dim) decides the
+ * bond in direction k, word 3 is the new value of the cluster whose root (minimum site index) is
+ * this site.
+ * Domain PACK (Ising): the 128 bits of one call serve S consecutive sites, index = site / S, with
+ * S = 4 in 2D and S = 2 in 3D; see ising_site_bits().  Domain TIE (Ising): index = site, word k
+ * settles bond k when its PACK field sits exactly on the threshold.
  * Domain INIT: start configuration, word 0.  Domain XYDIR: the XY direction of step t, word 0. */
-enum { DOM_SITE = 0, DOM_INIT = 2, DOM_XYDIR = 3 };
+enum { DOM_SITE = 0, DOM_PACK = 1, DOM_INIT = 2, DOM_XYDIR = 3, DOM_TIE = 4 };
 
 struct swo_ctx {
     int dim, L, model, q;
@@ -159,23 +163,71 @@ static uint32_t threshold32(double p)
     return (uint32_t)v;
 }
 
+/* Ising, reading 6: the random bits of site i at step t.  The 128 output bits of the PACK call
+ * number i / S are cut into S pieces of W = 128 / S bits, in word order; site i owns piece i % S
+ * (2D: word i % 4; 3D: words 2 (i % 2) [low] and 2 (i % 2) + 1 [high]).  Inside its piece, bond k
+ * has the F-bit field at bit offset k F, with F = (W - 1) / dim (15 in 2D, 21 in 3D), and the top
+ * bit of the piece is the new value of the cluster whose root is this site. */
+static int ising_field_bits(const swo_ctx *o) { return (o->dim == 2) ? 15 : 21; }
+
+static void ising_site_bits(const swo_ctx *o, size_t i, uint64_t t, uint32_t field[3], int *top_bit)
+{
+    const int S = (o->dim == 2) ? 4 : 2;
+    const int W = 128 / S;
+    const int F = ising_field_bits(o);
+    uint32_t w[4];
+    draw(o, (uint32_t)(i / (size_t)S), t, DOM_PACK, w);
+    uint64_t piece;
+    if (o->dim == 2) piece = w[i % 4];
+    else piece = (uint64_t)w[2 * (i % 2)] | ((uint64_t)w[2 * (i % 2) + 1] << 32);
+    for (int k = 0; k < o->dim; ++k) field[k] = (uint32_t)((piece >> (F * k)) & ((1u << F) - 1u));
+    *top_bit = (int)((piece >> (W - 1)) & 1u);
+}
+
+/* Ising bond decision with probability exactly P32 / 2^32 from an F-bit field: compare the field
+ * with the top F bits of P32; only if they are equal (probability 2^-F) the remaining 32 - F bits
+ * of P32 are compared with the top 32 - F bits of word k of the site's TIE call. */
+static int ising_bond_random(const swo_ctx *o, size_t i, uint64_t t, int k, uint32_t field, uint32_t P32)
+{
+    const int F = ising_field_bits(o);
+    const uint32_t Ptop = P32 >> (32 - F), Plow = P32 & ((1u << (32 - F)) - 1u);
+    if (field < Ptop) return 1;
+    if (field > Ptop) return 0;
+    uint32_t w[4];
+    draw(o, (uint32_t)i, t, DOM_TIE, w);
+    return (w[k] >> F) < Plow;
+}
+
 /* Sub-step (1): active-bond generation. */
 static void make_bonds(swo_ctx *o)
 {
     const uint64_t t = o->t;
     double nact = 0.0;
-    if (o->model == SWO_ISING || o->model == SWO_POTTS) {
-        double p = (o->model == SWO_ISING) ? -expm1(-2.0 * o->beta) : -expm1(-o->beta);
-        uint32_t P32 = threshold32(p);
+    if (o->model == SWO_ISING) {
+        uint32_t P32 = threshold32(-expm1(-2.0 * o->beta));
+        for (size_t i = 0; i < o->N; ++i) {
+            uint32_t field[3];
+            int top;
+            ising_site_bits(o, i, t, field, &top);
+            uint8_t b = 0;
+            for (int k = 0; k < o->dim; ++k) {
+                size_t j = nbr_plus(o, i, k);
+                if (o->s_ising[i] == o->s_ising[j] && ising_bond_random(o, i, t, k, field[k], P32)) {
+                    b |= (uint8_t)(1u << k);
+                    nact += 1.0;
+                }
+            }
+            o->bond[i] = b;
+        }
+    } else if (o->model == SWO_POTTS) {
+        uint32_t P32 = threshold32(-expm1(-o->beta));
         for (size_t i = 0; i < o->N; ++i) {
             uint32_t w[4];
             draw(o, (uint32_t)i, t, DOM_SITE, w);
             uint8_t b = 0;
             for (int k = 0; k < o->dim; ++k) {
                 size_t j = nbr_plus(o, i, k);
-                int equal = (o->model == SWO_ISING) ? (o->s_ising[i] == o->s_ising[j])
-                                                    : (o->s_potts[i] == o->s_potts[j]);
-                if (equal && w[k] < P32) { b |= (uint8_t)(1u << k); nact += 1.0; }
+                if (o->s_potts[i] == o->s_potts[j] && w[k] < P32) { b |= (uint8_t)(1u << k); nact += 1.0; }
             }
             o->bond[i] = b;
         }
@@ -248,7 +300,7 @@ static void label_clusters(swo_ctx *o)
 
 /* Sub-step (3): "All spins in each cluster are set randomly to +1 or -1" (reading
  * 5: a fresh value, not "flip with probability 1/2").  One draw per cluster at its root:
- * word 3 of the root's SITE call.  Potts: new state (w*q) >> 32.  XY (mirror
+ * Ising the top bit of the root's PACK piece, Potts and XY word 3 of the root's SITE call.  Potts: new state (w*q) >> 32.  XY (mirror
  * projection): if the top bit is set, reflect every spin of the cluster across the line
  * perpendicular to r: theta' = c - theta with c = (2 phi + pi) mod 2 pi, wrapped to [0, 2 pi]
  * -- two fp32 operations, done in float here exactly as the spec states them. */
@@ -258,9 +310,15 @@ static void flip_clusters(swo_ctx *o)
     const float two_pi_f = (float)TWO_PI;
     for (size_t i = 0; i < o->N; ++i) {
         uint32_t w[4];
+        if (o->model == SWO_ISING) {
+            uint32_t field[3];
+            int top;
+            ising_site_bits(o, o->label[i], t, field, &top);
+            o->s_ising[i] = top ? 1 : -1;
+            continue;
+        }
         draw(o, o->label[i], t, DOM_SITE, w);
-        if (o->model == SWO_ISING) o->s_ising[i] = (w[3] >> 31) ? 1 : -1;
-        else if (o->model == SWO_POTTS) o->s_potts[i] = (uint8_t)(((uint64_t)w[3] * (uint64_t)o->q) >> 32);
+        if (o->model == SWO_POTTS) o->s_potts[i] = (uint8_t)(((uint64_t)w[3] * (uint64_t)o->q) >> 32);
         else if (w[3] >> 31) {
             float th = o->crefl - o->s_xy[i];
             if (th < 0.0f) th = th + two_pi_f;

@@ -26,7 +26,7 @@
 namespace swk {
 
 enum { ISING = 0, POTTS = 1, XY = 2 };
-constexpr uint32_t DOM_SITE = 0u, DOM_INIT = 2u, DOM_XYDIR = 3u;
+constexpr uint32_t DOM_SITE = 0u, DOM_PACK = 1u, DOM_INIT = 2u, DOM_XYDIR = 3u, DOM_TIE = 4u;
 constexpr uint32_t FULL = 0xffffffffu;
 #ifndef SW_BL_THREADS_PER_SM
 #define SW_BL_THREADS_PER_SM 1536  // resident threads per SM k_bond_label is compiled for (register cap)
@@ -180,6 +180,20 @@ __device__ __forceinline__ void union_s(uint32_t *lab, uint32_t a, uint32_t b)
     }
 }
 
+// One pointer-jumping step for the 4 sites of a quad: r <- parent(r) where the previous step still
+// moved (r != prev); a site that has reached a fixed point (a root) issues no load, so roots and
+// their direct children cost no shared-memory wavefronts.
+__device__ __forceinline__ void jump4(volatile uint32_t *vl, uint4 &r, uint4 &prev)
+{
+    uint4 n;
+    n.x = (r.x != prev.x) ? vl[r.x] : r.x;
+    n.y = (r.y != prev.y) ? vl[r.y] : r.y;
+    n.z = (r.z != prev.z) ? vl[r.z] : r.z;
+    n.w = (r.w != prev.w) ? vl[r.w] : r.w;
+    prev = r;
+    r = n;
+}
+
 // ------------------------------------------------------------------------------------------------
 // k_init: seeded random start (the paper's device_function_spinset).
 // ------------------------------------------------------------------------------------------------
@@ -292,8 +306,10 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
         const uint32_t g = gx + L * (gy + L * gz);
         const bool rowend = (lane & (LPR - 1)) == LPR - 1;
         uint4 w[4];
+        if (MODEL != ISING) {
 #pragma unroll
-        for (int s = 0; s < 4; ++s) w[s] = philox4x32_10(g + s, p.t_lo, p.t_hi, DOM_SITE, p.k0, p.k1);
+            for (int s = 0; s < 4; ++s) w[s] = philox4x32_10(g + s, p.t_lo, p.t_hi, DOM_SITE, p.k0, p.k1);
+        }
         uint32_t bxn, byn, bzn = 0u, d;
         if (MODEL == XY) {
             // Wolff embedding: aligned iff a_i a_j > 0, p = 1 - exp(-2 beta a_i a_j)
@@ -324,28 +340,84 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
             }
             d = (w[0].w >> 31) | ((w[1].w >> 31) << 1) | ((w[2].w >> 31) << 2) | ((w[3].w >> 31) << 3);
         } else {
-            // a bond between equal neighbours is active with probability p (word < P32).
+            // a bond between equal neighbours is active with probability p.
             const uint8_t *sp = (const uint8_t *)p.spins;
             const uint32_t own = *reinterpret_cast<const uint32_t *>(sp + g);
             const uint32_t up = *reinterpret_cast<const uint32_t *>(sp + ((gy + 1 == L) ? g - L * (L - 1) : g + L));
             uint32_t nb = __shfl_down_sync(FULL, own, 1);
             if (rowend) nb = sp[(gx + 4 == L) ? g + 4 - L : g + 4];
-            const uint32_t P = p.P32;
-            bxn = eq4(own, __funnelshift_r(own, nb, 8)) &
-                  ((w[0].x < P) | ((w[1].x < P) << 1) | ((w[2].x < P) << 2) | ((w[3].x < P) << 3));
-            byn = eq4(own, up) & ((w[0].y < P) | ((w[1].y < P) << 1) | ((w[2].y < P) << 2) | ((w[3].y < P) << 3));
-            if (DIM == 3) {
-                const uint32_t fr = *reinterpret_cast<const uint32_t *>(sp + ((gz + 1 == L) ? g - LL * (L - 1) : g + LL));
-                bzn = eq4(own, fr) & ((w[0].z < P) | ((w[1].z < P) << 1) | ((w[2].z < P) << 2) | ((w[3].z < P) << 3));
-            }
-            if (MODEL == POTTS) {
+            uint32_t fr = 0u;
+            if (DIM == 3) fr = *reinterpret_cast<const uint32_t *>(sp + ((gz + 1 == L) ? g - LL * (L - 1) : g + LL));
+            uint32_t rnx, rny, rnz = 0u;  // nibbles: the random decision of each bond
+            if (MODEL == ISING) {
+                // Packed keying (reading 6): the 128 bits of one call serve S = 4 (2D) or 2 (3D)
+                // consecutive sites; a site's 32 / 64 bits hold one F-bit field per bond (F = 15 / 21)
+                // and, in the top bit, its cluster draw.  field < P32 >> (32 - F) decides the bond; a
+                // field equal to that value (probability 2^-F) is settled by the low bits of P32
+                // against a second call (domain TIE), so the probability is exactly P32 / 2^32.
+                constexpr int F = (DIM == 2) ? 15 : 21;
+                constexpr uint32_t FM = (1u << F) - 1u;
+                constexpr int SH2 = (DIM == 3) ? 2 * F - 32 : 0;  // field 2 inside the high word
+                const uint32_t Ptop = p.P32 >> (32 - F), Plow = p.P32 & ((1u << (32 - F)) - 1u);
+                uint32_t f0[4], f1[4], f2[4];
+                if (DIM == 2) {
+                    const uint4 c = philox4x32_10(g >> 2, p.t_lo, p.t_hi, DOM_PACK, p.k0, p.k1);
+                    const uint32_t cw[4] = {c.x, c.y, c.z, c.w};
+                    d = 0u;
+#pragma unroll
+                    for (int s = 0; s < 4; ++s) {
+                        f0[s] = cw[s] & FM; f1[s] = (cw[s] >> F) & FM; f2[s] = 0u;
+                        d |= (cw[s] >> 31) << s;
+                    }
+                } else {
+                    const uint4 c0 = philox4x32_10(g >> 1, p.t_lo, p.t_hi, DOM_PACK, p.k0, p.k1);
+                    const uint4 c1 = philox4x32_10((g >> 1) + 1u, p.t_lo, p.t_hi, DOM_PACK, p.k0, p.k1);
+                    const uint32_t lo[4] = {c0.x, c0.z, c1.x, c1.z}, hi[4] = {c0.y, c0.w, c1.y, c1.w};
+                    d = 0u;
+#pragma unroll
+                    for (int s = 0; s < 4; ++s) {
+                        f0[s] = lo[s] & FM;
+                        f1[s] = __funnelshift_r(lo[s], hi[s], F) & FM;
+                        f2[s] = (hi[s] >> SH2) & FM;
+                        d |= (hi[s] >> 31) << s;
+                    }
+                }
+                rnx = rny = 0u;
+                uint32_t tie = 0u;  // bit s + 4 k: field k of site s sits exactly on the threshold
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    rnx |= ((f0[s] - Ptop) >> 31) << s;   // fields and Ptop are < 2^21: the sign bit is "<"
+                    rny |= ((f1[s] - Ptop) >> 31) << s;
+                    tie |= (uint32_t)(f0[s] == Ptop) << s | (uint32_t)(f1[s] == Ptop) << (s + 4);
+                    if (DIM == 3) {
+                        rnz |= ((f2[s] - Ptop) >> 31) << s;
+                        tie |= (uint32_t)(f2[s] == Ptop) << (s + 8);
+                    }
+                }
+                if (tie) {
+#pragma unroll 1
+                    for (int s = 0; s < 4; ++s) {
+                        if ((tie >> s) & 0x111u) {
+                            const uint4 tw = philox4x32_10(g + s, p.t_lo, p.t_hi, DOM_TIE, p.k0, p.k1);
+                            if (((tie >> s) & 1u) && (tw.x >> F) < Plow) rnx |= 1u << s;
+                            if (((tie >> (s + 4)) & 1u) && (tw.y >> F) < Plow) rny |= 1u << s;
+                            if (((tie >> (s + 8)) & 1u) && (tw.z >> F) < Plow) rnz |= 1u << s;
+                        }
+                    }
+                }
+            } else {
+                const uint32_t P = p.P32;  // Potts: one call per site, word k < P32 decides bond k
+                rnx = (w[0].x < P) | ((w[1].x < P) << 1) | ((w[2].x < P) << 2) | ((w[3].x < P) << 3);
+                rny = (w[0].y < P) | ((w[1].y < P) << 1) | ((w[2].y < P) << 2) | ((w[3].y < P) << 3);
+                if (DIM == 3) rnz = (w[0].z < P) | ((w[1].z < P) << 1) | ((w[2].z < P) << 2) | ((w[3].z < P) << 3);
                 const unsigned qq = (unsigned)p.q;
                 d = 0u;
 #pragma unroll
                 for (int s = 0; s < 4; ++s) d |= (uint32_t)(((unsigned long long)w[s].w * qq) >> 32) << (s * db);
-            } else {
-                d = (w[0].w >> 31) | ((w[1].w >> 31) << 1) | ((w[2].w >> 31) << 2) | ((w[3].w >> 31) << 3);
             }
+            bxn = eq4(own, __funnelshift_r(own, nb, 8)) & rnx;
+            byn = eq4(own, up) & rny;
+            if (DIM == 3) bzn = eq4(own, fr) & rnz;
         }
         bnd[j] = bxn | (byn << 4) | (bzn << 8);
         drw[j] = d;
@@ -441,8 +513,9 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
         for (int j = 0; j < QPT; ++j) {
             const int li = (tid + j * NT) * 4;
             uint4 r = *reinterpret_cast<const uint4 *>(lab_s + li);
-            r.x = vl[r.x]; r.y = vl[r.y]; r.z = vl[r.z]; r.w = vl[r.w];
-            r.x = vl[r.x]; r.y = vl[r.y]; r.z = vl[r.z]; r.w = vl[r.w];
+            uint4 prev = make_uint4(li, li + 1, li + 2, li + 3);
+            jump4(vl, r, prev);
+            jump4(vl, r, prev);
             *reinterpret_cast<uint4 *>(lab_s + li) = r;
         }
         __syncthreads();
@@ -533,9 +606,10 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     for (int j = 0; j < QPT; ++j) {
         const int li = (tid + j * NT) * 4;
         uint4 r = *reinterpret_cast<const uint4 *>(lab_s + li);
+        uint4 prev = make_uint4(li, li + 1, li + 2, li + 3);
 #pragma unroll
         for (int k = 0; k < SW_BL_JUMPS; ++k) {
-            r.x = vlab[r.x]; r.y = vlab[r.y]; r.z = vlab[r.z]; r.w = vlab[r.w];
+            jump4(vlab, r, prev);
             if (k + 1 < SW_BL_JUMPS) *reinterpret_cast<uint4 *>(lab_s + li) = r;
         }
         const uint32_t dm = (1u << db) - 1u, d = drw[j];
@@ -667,31 +741,26 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
         const int li = (tid + j * NT) * 4;
         const uint32_t a0 = tile_base + li;
         const uint4 w4 = *reinterpret_cast<const uint4 *>(lab + a0);
+        // follow the parent words: at[s] is the node reached so far and pw[s] its word; the chase of a
+        // site ends at the node whose parent field is its own address, and that word's draw field is the
+        // cluster's new value
         uint32_t pw[4] = {w4.x, w4.y, w4.z, w4.w};
-        uint32_t tgt[4];
-        bool pend[4], same[4];
-#pragma unroll
-        for (int s = 0; s < 4; ++s) {
-            tgt[s] = pw[s] >> db;
-            same[s] = s > 0 && tgt[s] == tgt[s - 1];
-            pend[s] = tgt[s] != a0 + s && !same[s];
-        }
-        while (pend[0] | pend[1] | pend[2] | pend[3]) {
+        uint32_t at[4] = {a0, a0 + 1u, a0 + 2u, a0 + 3u};
+        for (;;) {
+            uint32_t moving = 0u;
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
-                if (pend[s]) {
-                    const uint32_t nw = __ldg(lab + tgt[s]);
-                    const uint32_t np = nw >> db;
-                    ++chase_hops;
-                    if (np == tgt[s]) { pw[s] = nw; pend[s] = false; }
-                    else tgt[s] = np;
+                const uint32_t par = pw[s] >> db;
+                if (par != at[s]) {
+                    at[s] = par;
+                    pw[s] = __ldg(lab + par);
+                    moving = 1u;
                 }
             }
+            if (!moving) break;
+            ++chase_hops;
         }
         __syncwarp();
-#pragma unroll
-        for (int s = 1; s < 4; ++s)
-            if (same[s]) pw[s] = pw[s - 1];
 
         const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
         const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));

@@ -180,18 +180,30 @@ def test_determinism_and_step_batching():
     assert not np.array_equal(a.spins(), c.spins())
 
 
-def test_ising_equals_potts_q2():
-    """R1: Ising(beta) == Potts(q=2, 2 beta) bit for bit under s = 2k - 1."""
-    sw, _ = _mods()
-    beta = 1.0 / TC2
-    a = sw.SwendsenWang(2, 128, 0, 0, beta, seed=4, record_bonds=True)
-    b = sw.SwendsenWang(2, 128, 1, 2, 2.0 * beta, seed=4, record_bonds=True)
-    for t in range(20):
-        a.step(1)
-        b.step(1)
-        assert np.array_equal(a.spins(), 2 * b.spins().astype(np.int8) - 1)
-        assert np.array_equal(a.labels(), b.labels())
-        assert np.array_equal(a.bonds(), b.bonds())
+@pytest.mark.parametrize("dim,L", [(2, 64), (3, 32)])
+def test_ising_forced_tie_parity(dim, L):
+    """Packed Ising keying (reading 6): a bond whose F-bit field equals the top F bits of
+    the threshold is settled by the TIE call.  That has probability 2^-F per bond, so the case is
+    forced: beta is chosen so that the threshold's top part equals a field that does occur."""
+    sw, orc = _mods()
+    from paper_1403_7560_b200 import inputs
+    seed, t0, N = 21, 7, L ** dim
+    S, W = (4, 32) if dim == 2 else (2, 64)
+    F = (W - 1) // dim
+    for site, k in [(3, 0), (N // 3, dim - 1), (N - 2, 1)]:
+        w = orc.philox4x32_10([site // S, t0, 0, 1], [seed, 0])
+        piece = w[site % 4] if dim == 2 else (w[2 * (site % 2)] | (w[2 * (site % 2) + 1] << 32))
+        v = (piece >> (F * k)) & ((1 << F) - 1)
+        beta = -0.5 * math.log1p(-(v + 0.5) / (1 << F))
+        g = sw.SwendsenWang(dim, L, 0, 0, beta, seed=seed, record_bonds=True)
+        o = orc.Oracle(dim, L, 0, 0, beta, seed)
+        cold = inputs.aligned_spins(0, N)
+        g.set_spins(cold, t0)
+        o.set_spins(cold, t0)
+        g.step(1)
+        o.step(1)
+        _compare_step(g, o, f"forced tie dim{dim} site {site} dir {k}")
+        g.close()
 
 
 def test_state_errors():

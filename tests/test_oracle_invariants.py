@@ -88,17 +88,61 @@ def test_determinism_and_state_injection():
     assert not np.array_equal(a.spins(), d.spins())
 
 
-def test_ising_equals_potts_q2_bit_for_bit():
-    """R1: Ising(beta) == Potts(q = 2, 2 beta) under s = 2k - 1 (same thresholds, same words)."""
-    for dim, L, beta in [(2, 16, 0.4406868), (3, 6, 0.2216544)]:
-        a = so.Oracle(dim, L, so.ISING, 0, beta, seed=9)
-        b = so.Oracle(dim, L, so.POTTS, 2, 2.0 * beta, seed=9)
-        assert np.array_equal(a.spins(), 2 * b.spins().astype(np.int8) - 1)
-        for _ in range(20):
-            a.step(1)
-            b.step(1)
-            assert np.array_equal(a.bonds(), b.bonds()) and np.array_equal(a.labels(), b.labels())
-            assert np.array_equal(a.spins(), 2 * b.spins().astype(np.int8) - 1)
+def _ising_bits_restated(dim, i, t, seed):
+    """DESIGN.md reading 6 written out again with the Philox routine as a library step: the F-bit
+    bond fields and the top bit of site i's piece of PACK call i // S."""
+    S, W = (4, 32) if dim == 2 else (2, 64)
+    F = (W - 1) // dim
+    w = so.philox4x32_10([i // S, t & 0xffffffff, t >> 32, 1], [seed & 0xffffffff, seed >> 32])
+    piece = w[i % 4] if dim == 2 else (w[2 * (i % 2)] | (w[2 * (i % 2) + 1] << 32))
+    return [(piece >> (F * k)) & ((1 << F) - 1) for k in range(dim)], (piece >> (W - 1)) & 1, F
+
+
+@pytest.mark.parametrize("dim,L", [(2, 32), (3, 8)])
+def test_ising_packed_keying_and_tie_rule(dim, L):
+    """Reading 6 (packed Ising keying): every bond decision and every cluster value of the oracle
+    against the rule restated here, including bonds whose field sits exactly on the threshold
+    (settled by the TIE call).  A tie has probability 2^-F, so it is forced: the threshold's top
+    part is set to a field value that does occur at t = 0 (beta is free)."""
+    seed, N = 11, L ** dim
+    F = (31 if dim == 2 else 63) // dim
+    cold = np.ones(N, dtype=np.int8)
+    ties = 0
+    for site, k0 in [(5, 0), (N // 2 + 3, dim - 1), (N - 1, 1), (17, 0)]:
+        v = _ising_bits_restated(dim, site, 0, seed)[0][k0]
+        p_bond = (v + 0.5) / (1 << F)          # Ptop = v, Plow = half its range
+        beta = -0.5 * math.log1p(-p_bond)
+        P32 = int(math.floor(-math.expm1(-2.0 * beta) * 4294967296.0))
+        Ptop, Plow = P32 >> (32 - F), P32 & ((1 << (32 - F)) - 1)
+        assert Ptop == v and 0 < Plow < (1 << (32 - F))
+        o = so.Oracle(dim, L, so.ISING, 0, beta, seed=seed)
+        o.set_spins(cold, 0)          # every pair is aligned: the bond byte is the random decision
+        o.step(1)
+        bonds, labels, spins = o.bonds(), o.labels(), o.spins()
+        for i in range(N):
+            fields, top, _ = _ising_bits_restated(dim, i, 0, seed)
+            for k in range(dim):
+                if fields[k] == Ptop:
+                    ties += 1
+                    tw = so.philox4x32_10([i, 0, 0, 4], [seed, 0])
+                    want = (tw[k] >> F) < Plow
+                else:
+                    want = fields[k] < Ptop
+                assert bool((bonds[i] >> k) & 1) == want, (site, i, k)
+        for r in np.unique(labels)[:64]:
+            _, top, _ = _ising_bits_restated(dim, int(r), 0, seed)
+            assert (spins[labels == r] == (1 if top else -1)).all()
+    assert ties >= 4, "the tie rule was not exercised"
+
+
+def test_ising_threshold_split_is_exact():
+    """P(active) = Ptop / 2^F + 2^-F Plow / 2^(32-F) must equal P32 / 2^32 for every P32."""
+    from fractions import Fraction
+    rng = np.random.default_rng(3)
+    for F in (15, 21):
+        for P32 in [0, 1, 2 ** 32 - 1, 2515933809, 1537996873] + [int(x) for x in rng.integers(0, 2 ** 32, size=50)]:
+            Ptop, Plow = P32 >> (32 - F), P32 & ((1 << (32 - F)) - 1)
+            assert Fraction(Ptop, 2 ** F) + Fraction(1, 2 ** F) * Fraction(Plow, 2 ** (32 - F)) == Fraction(P32, 2 ** 32)
 
 
 def test_thresholds_of_the_configs():
