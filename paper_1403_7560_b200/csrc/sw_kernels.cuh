@@ -358,7 +358,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                 constexpr int F = (DIM == 2) ? 15 : 21;
                 constexpr uint32_t FM = (1u << F) - 1u;
                 constexpr int SH2 = (DIM == 3) ? 2 * F - 32 : 0;  // field 2 inside the high word
-                const uint32_t Ptop = p.P32 >> (32 - F), Plow = p.P32 & ((1u << (32 - F)) - 1u);
+                const uint32_t Ptop = p.P32 >> (32 - F);
                 uint32_t f0[4], f1[4], f2[4];
                 if (DIM == 2) {
                     const uint4 c = philox4x32_10(g >> 2, p.t_lo, p.t_hi, DOM_PACK, p.k0, p.k1);
@@ -382,26 +382,34 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                         d |= (hi[s] >> 31) << s;
                     }
                 }
+                // d = field - Ptop (both < 2^21): the sign bit of d is "field < Ptop", and d == 0 is a tie.
+                // Sign bits are shifted into the nibbles with one funnel shift each (sites 3..0), and the
+                // minimum of all d tells whether any field of the quad sits on the threshold.
                 rnx = rny = 0u;
-                uint32_t tie = 0u;  // bit s + 4 k: field k of site s sits exactly on the threshold
+                uint32_t dmin = 0xffffffffu;
 #pragma unroll
-                for (int s = 0; s < 4; ++s) {
-                    rnx |= ((f0[s] - Ptop) >> 31) << s;   // fields and Ptop are < 2^21: the sign bit is "<"
-                    rny |= ((f1[s] - Ptop) >> 31) << s;
-                    tie |= (uint32_t)(f0[s] == Ptop) << s | (uint32_t)(f1[s] == Ptop) << (s + 4);
+                for (int s = 3; s >= 0; --s) {
+                    const uint32_t d0 = f0[s] - Ptop, d1 = f1[s] - Ptop;
+                    rnx = __funnelshift_l(d0, rnx, 1);
+                    rny = __funnelshift_l(d1, rny, 1);
+                    dmin = min(dmin, min(d0, d1));
                     if (DIM == 3) {
-                        rnz |= ((f2[s] - Ptop) >> 31) << s;
-                        tie |= (uint32_t)(f2[s] == Ptop) << (s + 8);
+                        const uint32_t d2 = f2[s] - Ptop;
+                        rnz = __funnelshift_l(d2, rnz, 1);
+                        dmin = min(dmin, d2);
                     }
                 }
-                if (tie) {
-#pragma unroll 1
+                if (dmin == 0u) {  // probability 12 x 2^-21 per quad (3D), 8 x 2^-15 (2D)
+                    // fully unrolled: the field arrays are only ever indexed statically (registers)
+                    const uint32_t Plow = p.P32 & ((1u << (32 - F)) - 1u);
+#pragma unroll
                     for (int s = 0; s < 4; ++s) {
-                        if ((tie >> s) & 0x111u) {
+                        const bool t0 = f0[s] == Ptop, t1 = f1[s] == Ptop, t2 = DIM == 3 && f2[s] == Ptop;
+                        if (t0 || t1 || t2) {
                             const uint4 tw = philox4x32_10(g + s, p.t_lo, p.t_hi, DOM_TIE, p.k0, p.k1);
-                            if (((tie >> s) & 1u) && (tw.x >> F) < Plow) rnx |= 1u << s;
-                            if (((tie >> (s + 4)) & 1u) && (tw.y >> F) < Plow) rny |= 1u << s;
-                            if (((tie >> (s + 8)) & 1u) && (tw.z >> F) < Plow) rnz |= 1u << s;
+                            if (t0 && (tw.x >> F) < Plow) rnx |= 1u << s;
+                            if (t1 && (tw.y >> F) < Plow) rny |= 1u << s;
+                            if (t2 && (tw.z >> F) < Plow) rnz |= 1u << s;
                         }
                     }
                 }
