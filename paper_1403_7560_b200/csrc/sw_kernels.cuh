@@ -37,6 +37,9 @@ constexpr uint32_t FULL = 0xffffffffu;
 #ifndef SW_BL_ROUNDS
 #define SW_BL_ROUNDS 1  // uniform hook + flatten rounds before the general union-find loop
 #endif
+#ifndef SW_BL_HOOK_LOOP
+#define SW_BL_HOOK_LOOP 1  // 3D hook round: 1 = loop over the active bonds, 0 = predicated code over all bond slots
+#endif
 #ifndef SW_BL_JUMPS
 #define SW_BL_JUMPS 2  // pointer-jumping rounds over the tile-local forest before it is stored
 #endif
@@ -491,6 +494,23 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     const uint32_t lab_sa = (uint32_t)__cvta_generic_to_shared(lab_s);
 #pragma unroll 1
     for (int round = 0; round < SW_BL_ROUNDS; ++round) {
+        if (SW_BL_HOOK_LOOP && DIM == 3) {
+            // one iteration per active bond of the thread (trip count = the largest popcount in the
+            // warp): at 3D densities (a quarter of the bond slots active) this beats the predicated code
+            uint32_t todo = work;
+            work = 0u;
+            while (__any_sync(FULL, todo != 0u)) {
+                if (todo) {
+                    const int k = __ffs(todo) - 1;
+                    todo &= todo - 1u;
+                    const uint32_t a = (uint32_t)((tid + (k / WB) * NT) * 4 + (k & 3));
+                    const uint32_t b = a + (((k % WB) & 4) ? (uint32_t)(TX * TY) : (uint32_t)TX);
+                    const uint32_t pa = lab_s[a], pb = lab_s[b];
+                    const uint32_t hi = max(pa, pb), lo = min(pa, pb);
+                    if (hi != lo && atomicCAS(&lab_s[hi], hi, lo) != hi) work |= 1u << k;
+                }
+            }
+        } else {
 #pragma unroll
         for (int j = 0; j < QPT; ++j) {
             const int li = (tid + j * NT) * 4;
@@ -514,6 +534,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                 }
                 work = (work & ~(0xfu << (j * WB + 4 * dir))) | (left << (j * WB + 4 * dir));
             }
+        }
         }
         __syncthreads();
         volatile uint32_t *vl = lab_s;
