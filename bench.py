@@ -63,6 +63,11 @@ def kernel_bytes_per_site(model):
     return {"k_bond_label": sp + 4, "k_merge": 0, "k_flip": 4 + sp + (sp if model == 2 else 0)}
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the one
+# `ncu --set full` capture summarised in profiles/r01_final_ncu_full_C4.md (config -> kernel -> bytes).
+NCU_TRAFFIC = {"C4": {"k_bond_label": 141.2e6 + 1.15e9, "k_merge": 632.9e6 + 120.8e6, "k_flip": 537.9e6 + 120.2e6}}
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons sampled while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -265,7 +270,9 @@ def run_ours(args):
     achieved = kb[name] * n_sites / (kms[dom] * 1e-3) / 1e9 if kms[dom] > 0 else 0.0
     step_gbs = floor_bytes_per_site(cfg["model"]) * n_sites / (ms * 1e-3) / 1e9
     out["roofline"] = {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                       "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                       "frac": achieved / peak, "traffic": NCU_TRAFFIC.get(args.config, {}).get(name),
+                       "traffic_source": "profiles/r01_final_ncu_full_C4.md (ncu --set full, per launch)"
+                       if args.config in NCU_TRAFFIC else None, "peak_source": peak_src,
                        "kernel_ms": dict(zip(KERNELS, kms)),
                        "kernel_share": {k: v / max(sum(kms), 1e-12) for k, v in zip(KERNELS, kms)},
                        "bytes_per_site": kb,
