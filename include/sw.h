@@ -19,10 +19,14 @@
  *   bond byte    bit k = the bond from site i to its +e_k neighbour is active;
  *   label        minimum linear site index of the site's cluster (what label equivalence with
  *                atomicMin from label = index converges to);
- *   randoms      Philox4x32-10, key = (seed low, seed high), counter = (site, t low, t high,
- *                domain); domain 0: word k decides bond k of the site, word 3 is the new value of
- *                the cluster rooted at the site; domain 2: start configuration; domain 3: XY
- *                direction of step t.  t = 0-based index of the step being executed.
+ *   randoms      Philox4x32-10, key = (seed low, seed high), counter = (index, t low, t high,
+ *                domain), t = 0-based index of the step being executed.  Potts, XY: domain 0,
+ *                index = site, word k decides bond k of the site, word 3 is the new value of the
+ *                cluster rooted at the site.  Ising: domain 1, one call serves 4 (2D) or 2 (3D)
+ *                consecutive sites with 15- / 21-bit fields per bond and the cluster value in the
+ *                top bit of the site's piece; a field equal to the top bits of the threshold is
+ *                settled by a second call (domain 4), so P(bond) is exactly floor(p 2^32) / 2^32.
+ *                Domain 2: start configuration; domain 3: XY direction of step t.
  *
  * Pointers: `sw_ctx *` is an opaque HOST pointer owned by the library.  All `host_*` arguments
  * are HOST pointers owned by the caller.  `device_workspace` (sw_create_in) is a DEVICE pointer
@@ -125,8 +129,9 @@ int sw_force_xy_phi(sw_ctx *c, int enable, double phi);
  * when the context was switched to counting mode with sw_set_counting(c, 1), which makes the
  * kernels slower.  out[0] = tile-face bond slots examined, out[1] = active ones (unions attempted),
  * out[2] = unions that linked two roots, out[3] = union retries (lost atomicCAS), out[4] = total
- * find hops in the merge, out[5] = max find hops of one union, out[6] = total root-chase hops in
- * the flip kernel, out[7] = max chase hops of one thread (16 sites). */
+ * find hops in the merge, out[5] = max find hops of one union, out[6] = rounds of the root-chase
+ * loop in the flip kernel summed over threads (a round advances up to 4 sites by one parent), out[7] =
+ * the largest such sum of one thread (16 sites). */
 int sw_set_counting(sw_ctx *c, int enable);
 int sw_get_label_stats(sw_ctx *c, uint64_t *host_out, int n);
 
