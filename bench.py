@@ -118,7 +118,7 @@ def load_peak():
 # ---------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------
-DEFAULT_BURN_IN = {"C1": 200, "C2": 200, "C3": 200, "C4": 150, "C5": 100}
+DEFAULT_BURN_IN = {"C1": 200, "C2": 200, "C3": 200, "C4": 150, "C5": 100, "X1": 100, "X2": 100}
 L2_BYTES = 126 * 2 ** 20
 
 
@@ -229,7 +229,7 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    cfg = inputs.CONFIGS[args.config]
+    cfg = {**inputs.CONFIGS, **inputs.EXTRA_CONFIGS}[args.config]
     n_sites = cfg["L"] ** cfg["dim"]
     burn = args.burn_in if args.burn_in >= 0 else DEFAULT_BURN_IN[args.config]
     warm = max(args.warmup, 3)
@@ -279,13 +279,26 @@ def run_ours(args):
                        "step": {"floor_bytes_per_site": floor_bytes_per_site(cfg["model"]), "achieved": step_gbs,
                                 "frac": step_gbs / peak}}
     if rank == 0 and not args.no_extras:
+        # the paper's second row (Table 1): update + measurement of E and M every step,
+        # through sw_run_series (per-step sums stay on the device)
+        ns = max(3, min(args.steps, 20))
+        g.run_series(3)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g.run_series(ns)
+        e1.record()
+        torch.cuda.synchronize()
+        ms_meas = e0.elapsed_time(e1) / ns
+        out["with_measurement"] = {"ms_per_step": ms_meas, "value": n_sites / (ms_meas * 1e-3), "unit": UNIT,
+                                   "what": "sw_run_series: every step followed by k_measure (E, and M for XY) and a snapshot"}
         out["e2e"] = measure_e2e(sw, torch, g, cfg, max(3, min(args.steps, 10)))
         if world == 1:
             spins, t = g.spins(), g.t
             out["cpu_baseline"] = oracle_baseline(cfg, spins, t)
             del spins
             others = {}
-            for name_c, c in inputs.CONFIGS.items():
+            for name_c, c in list(inputs.CONFIGS.items()) + list(inputs.EXTRA_CONFIGS.items()):
                 if name_c == args.config:
                     continue
                 g2, ms2, kms2, fl2 = time_config(sw, torch, c, args.seed, DEFAULT_BURN_IN[name_c], 3,
@@ -313,7 +326,7 @@ def run_reference(args):
         return
     from oracle import sw_oracle as orc
     from paper_1403_7560_b200 import inputs
-    cfg = dict(inputs.CONFIGS[args.config])
+    cfg = dict({**inputs.CONFIGS, **inputs.EXTRA_CONFIGS}[args.config])
     budget = 150.0
     warm = max(args.warmup, 3)
     cands = [cfg["L"]] + ([256, 128, 64, 32] if cfg["dim"] == 3 else [2048, 1024, 512, 256, 128, 64])

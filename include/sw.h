@@ -82,8 +82,17 @@ int sw_step(sw_ctx *c, int n);
  *   Potts: E = number of unequal nearest-neighbour pairs (Eq. 2), M2 = (q sum_k n_k^2 - N^2)/(q-1)
  *          (Eq. 5), M = sqrt(M2), M4 = M2^2.
  *   XY:    E = -sum_<ij> cos(theta_i - theta_j) (Eq. 3), M = |sum_i (cos, sin)|, M2, M4 likewise.
- * Averages, the specific heat and the moment ratio (Eq. 6) are the caller's job. */
+ * Averages, the specific heat and the moment ratio (Eq. 6) are the caller's job.  Spins injected
+ * with sw_set_spins must lie in the model's range (Ising +-1, Potts 0..q-1): the sums are taken
+ * from byte-equality counts. */
 int sw_observables(sw_ctx *c, double *host_E, double *host_M, double *host_M2, double *host_M4);
+
+/* n SW steps with the observables of the configuration after EVERY step (the paper's measurement
+ * loop): the per-step sums stay on the device and are
+ * copied out once at the end, so there is no host round trip per step.  host_E .. host_M4 are HOST
+ * arrays of n doubles each (any may be NULL) with the same meaning as in sw_observables.  Needs
+ * n x (5 + q) x 8 bytes of scratch device memory for the call (SW_ENOMEM if that fails). */
+int sw_run_series(sw_ctx *c, int n, double *host_E, double *host_M, double *host_M2, double *host_M4);
 
 /* Destroy the context (synchronises its stream first).  NULL is a no-op. */
 int sw_destroy(sw_ctx *c);

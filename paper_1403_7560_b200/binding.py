@@ -39,6 +39,7 @@ def lib():
     L.sw_workspace_bytes.restype = sz
     L.sw_step.argtypes = [vp, i32]
     L.sw_observables.argtypes = [vp] + [C.POINTER(dbl)] * 4
+    L.sw_run_series.argtypes = [vp, i32, vp, vp, vp, vp]
     L.sw_destroy.argtypes = [vp]
     L.sw_last_error.restype = C.c_char_p
     L.sw_num_sites.argtypes = [vp]
@@ -137,6 +138,12 @@ class SwendsenWang:
         v = [C.c_double() for _ in range(4)]
         _check(lib().sw_observables(self._h, *[C.byref(x) for x in v]))
         return tuple(x.value for x in v)
+
+    def run_series(self, n):
+        """n steps, observables after every step (device-side series, one copy at the end)."""
+        out = {k: np.empty(n, dtype=np.float64) for k in ("E", "M", "M2", "M4")}
+        _check(lib().sw_run_series(self._h, int(n), *[out[k].ctypes.data for k in ("E", "M", "M2", "M4")]))
+        return out
 
     def counts(self):
         n = self.q if self.model == POTTS else 1

@@ -10,6 +10,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 using namespace swk;
 
@@ -212,9 +213,15 @@ void launch_init(sw_ctx *c)
 template <int DIM, int MODEL>
 void launch_measure_dm(sw_ctx *c, bool with_m)
 {
-    const unsigned g = (unsigned)(c->N / 256);
-    if (with_m) k_measure<DIM, MODEL, true><<<g, 256, 0, c->stream>>>(c->p);
-    else k_measure<DIM, MODEL, false><<<g, 256, 0, c->stream>>>(c->p);
+    if (MODEL == XY) {
+        const unsigned g = (unsigned)(c->N / 256);
+        if (with_m) k_measure<DIM, MODEL, true><<<g, 256, 0, c->stream>>>(c->p);
+        else k_measure<DIM, MODEL, false><<<g, 256, 0, c->stream>>>(c->p);
+    } else {
+        const unsigned g = (unsigned)(c->N / 1024);  // four sites per thread
+        if (with_m) k_measure4<DIM, MODEL, true><<<g, 256, 0, c->stream>>>(c->p);
+        else k_measure4<DIM, MODEL, false><<<g, 256, 0, c->stream>>>(c->p);
+    }
 }
 
 void launch_measure(sw_ctx *c, bool with_m)
@@ -242,6 +249,30 @@ int refresh_observables(sw_ctx *c)
     SW_CUDA(c, cudaGetLastError());
     c->E_fresh = c->M_fresh = true;
     return SW_OK;
+}
+
+// Extensive observables from the accumulator head (E_int, E_xy, M_int, mx, my, n_k[q]).
+void sums_to_observables(const sw_ctx *c, const unsigned long long *w, double &e, double &m, double &m2)
+{
+    double dv[5];
+    std::memcpy(dv, w, sizeof(dv));
+    if (c->model == SW_ISING) {
+        e = (double)(long long)w[0];
+        m = (double)(long long)w[2];
+        m2 = m * m;
+    } else if (c->model == SW_POTTS) {
+        // Eq. (5), PAPER.md:154: M^2 = (q sum_k n_k^2 - N^2) / (q - 1)
+        double s2 = 0.0;
+        for (int k = 0; k < c->q; ++k) s2 += (double)w[5 + k] * (double)w[5 + k];
+        const double Nd = (double)c->N;
+        e = (double)(long long)w[0];
+        m2 = ((double)c->q * s2 - Nd * Nd) / (double)(c->q - 1);
+        m = std::sqrt(m2);
+    } else {
+        e = dv[1];
+        m2 = dv[3] * dv[3] + dv[4] * dv[4];
+        m = std::sqrt(m2);
+    }
 }
 
 int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, uint64_t seed,
@@ -441,28 +472,60 @@ int sw_observables(sw_ctx *c, double *E, double *M, double *M2, double *M4)
     SW_CUDA(c, cudaMemcpyAsync(&h, c->p.acc, offsetof(Acc, stats), cudaMemcpyDeviceToHost, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
     double e, m, m2;
-    if (c->model == SW_ISING) {
-        e = (double)(long long)h.E_int;
-        m = (double)(long long)h.M_int;
-        m2 = m * m;
-    } else if (c->model == SW_POTTS) {
-        // Eq. (5), PAPER.md:154: M^2 = (q sum_k n_k^2 - N^2) / (q - 1)
-        double s2 = 0.0;
-        for (int k = 0; k < c->q; ++k) s2 += (double)h.nk[k] * (double)h.nk[k];
-        const double Nd = (double)c->N;
-        e = (double)(long long)h.E_int;
-        m2 = ((double)c->q * s2 - Nd * Nd) / (double)(c->q - 1);
-        m = std::sqrt(m2);
-    } else {
-        e = h.E_xy;
-        m2 = h.mx * h.mx + h.my * h.my;
-        m = std::sqrt(m2);
-    }
+    sums_to_observables(c, (const unsigned long long *)&h, e, m, m2);
     if (E) *E = e;
     if (M) *M = m;
     if (M2) *M2 = m2;
     if (M4) *M4 = m2 * m2;
     return SW_OK;
+}
+
+int sw_run_series(sw_ctx *c, int n, double *E, double *M, double *M2, double *M4)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (n < 0) return fail(SW_EINVAL, "n < 0");
+    if (n == 0) return SW_OK;
+    // per step one record of 5 + q 64-bit words = the head of Acc (E_int, E_xy, M_int, mx, my, n_k)
+    const int words = 5 + c->q;
+    unsigned long long *dser = nullptr;
+    cudaError_t e = cudaMalloc(&dser, (size_t)n * words * 8);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SW_ENOMEM, "sw_run_series: cudaMalloc of the series buffer failed"); }
+    for (int s = 0; s < n && rc == SW_OK; ++s) {
+        rc = sw_step(c, 1);
+        if (rc == SW_OK) rc = refresh_observables(c);
+        if (rc == SW_OK) {
+            k_snapshot<<<1, 288, 0, c->stream>>>(c->p.acc, dser + (size_t)s * words, words);
+            if (cudaGetLastError() != cudaSuccess) rc = fail(SW_ECUDA, "k_snapshot launch");
+        }
+    }
+    unsigned long long *hser = nullptr;
+    if (rc == SW_OK) {
+        hser = (unsigned long long *)std::malloc((size_t)n * words * 8);
+        if (!hser) rc = fail(SW_ENOMEM, "sw_run_series: host buffer");
+    }
+    if (rc == SW_OK) {
+        e = cudaMemcpyAsync(hser, dser, (size_t)n * words * 8, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) rc = cuda_fail(c, e, "sw_run_series copy");
+    } else {
+        cudaStreamSynchronize(c->stream);
+    }
+    if (rc == SW_OK) {
+        std::vector<unsigned long long> rec(5 + 256, 0ull);
+        for (int s = 0; s < n; ++s) {
+            std::memcpy(rec.data(), hser + (size_t)s * words, (size_t)words * 8);
+            double ev, m, m2;
+            sums_to_observables(c, rec.data(), ev, m, m2);
+            if (E) E[s] = ev;
+            if (M) M[s] = m;
+            if (M2) M2[s] = m2;
+            if (M4) M4[s] = m2 * m2;
+        }
+    }
+    std::free(hser);
+    cudaFree(dser);
+    return rc;
 }
 
 int sw_destroy(sw_ctx *c)

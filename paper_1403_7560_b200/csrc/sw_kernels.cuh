@@ -40,6 +40,9 @@ constexpr uint32_t FULL = 0xffffffffu;
 #ifndef SW_BL_HOOK_LOOP
 #define SW_BL_HOOK_LOOP 1  // 3D hook round: 1 = loop over the active bonds, 0 = predicated code over all bond slots
 #endif
+#ifndef SW_BL_MIDJUMPS
+#define SW_BL_MIDJUMPS 2  // pointer-jumping steps after a hook round
+#endif
 #ifndef SW_BL_JUMPS
 #define SW_BL_JUMPS 2  // pointer-jumping rounds over the tile-local forest before it is stored
 #endif
@@ -551,8 +554,8 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
             const int li = (tid + j * NT) * 4;
             uint4 r = *reinterpret_cast<const uint4 *>(lab_s + li);
             uint4 prev = make_uint4(li, li + 1, li + 2, li + 3);
-            jump4(vl, r, prev);
-            jump4(vl, r, prev);
+#pragma unroll
+            for (int k = 0; k < SW_BL_MIDJUMPS; ++k) jump4(vl, r, prev);
             *reinterpret_cast<uint4 *>(lab_s + li) = r;
         }
         __syncthreads();
@@ -962,6 +965,78 @@ __global__ void __launch_bounds__(256) k_measure(const Params p)
             if (tid < p.q && hist_s[tid]) atomicAdd(&p.acc->nk[tid], hist_s[tid]);
         }
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// k_measure4 (Ising, Potts): as k_measure, four consecutive sites per thread.  The spin words of the
+// quad and of its +x / +y / +z neighbours give byte-equality masks; with spins in the model's range
+// the energy is a popcount: Ising -sum s_i s_j = (#pairs - 2 #equal), Potts #unequal pairs.
+// ------------------------------------------------------------------------------------------------
+template <int DIM, int MODEL, bool WITH_M>
+__global__ void __launch_bounds__(256) k_measure4(const Params p)
+{
+    __shared__ uint32_t hist_s[256];
+    __shared__ int red_s[2][8];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t L = p.L, LL = L * L;
+    const uint32_t g = (blockIdx.x * 256u + tid) * 4u;  // N is a multiple of 1024
+    if (MODEL == POTTS && WITH_M) {
+        hist_s[tid] = 0u;
+        __syncthreads();
+    }
+    uint32_t x, y, z;
+    decode(p, g, x, y, z);
+    const uint8_t *sp = (const uint8_t *)p.spins;
+    const uint32_t own = *reinterpret_cast<const uint32_t *>(sp + g);
+    const uint32_t nb = sp[(x + 4 == L) ? g + 4 - L : g + 4];
+    const uint32_t up = *reinterpret_cast<const uint32_t *>(sp + ((y + 1 == L) ? g - L * (L - 1) : g + L));
+    int equal = __popc(eq4(own, __funnelshift_r(own, nb, 8))) + __popc(eq4(own, up));
+    if (DIM == 3) {
+        const uint32_t fr = *reinterpret_cast<const uint32_t *>(sp + ((z + 1 == L) ? g - LL * (L - 1) : g + LL));
+        equal += __popc(eq4(own, fr));
+    }
+    int e = (MODEL == ISING) ? 4 * DIM - 2 * equal : 4 * DIM - equal;
+    int m = 0;
+    if (WITH_M) {
+        if (MODEL == ISING) {
+            m = 4 - 2 * __popc(own & 0x80808080u);  // +1 = 0x01, -1 = 0xff
+        } else if (p.q <= 8) {
+            uint32_t lo = 0u, hi = 0u;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const uint32_t v = (own >> (8 * s)) & 0xffu, inc = 1u << ((v & 3u) * 8u);
+                if (v & 4u) hi += inc; else lo += inc;
+            }
+            for (int k = 0; k < p.q; ++k) {
+                const uint32_t c = ((k < 4 ? lo : hi) >> ((k & 3) * 8)) & 0xffu;
+                const uint32_t w = __reduce_add_sync(FULL, c);
+                if (lane == 0 && w) atomicAdd(&hist_s[k], w);
+            }
+        } else {
+#pragma unroll
+            for (int s = 0; s < 4; ++s) atomicAdd(&hist_s[(own >> (8 * s)) & 0xffu], 1u);
+        }
+    }
+    e = __reduce_add_sync(FULL, e);
+    m = __reduce_add_sync(FULL, m);
+    if (lane == 0) { red_s[0][warp] = e; red_s[1][warp] = m; }
+    __syncthreads();
+    if (tid == 0) {
+        long long es = 0, ms = 0;
+        for (int w = 0; w < 8; ++w) { es += red_s[0][w]; ms += red_s[1][w]; }
+        atomicAdd(&p.acc->E_int, (unsigned long long)es);
+        if (WITH_M && MODEL == ISING) atomicAdd(&p.acc->M_int, (unsigned long long)ms);
+    }
+    if (MODEL == POTTS && WITH_M) {
+        if (tid < p.q && hist_s[tid]) atomicAdd(&p.acc->nk[tid], (unsigned long long)hist_s[tid]);
+    }
+}
+
+// k_snapshot: copy the head of the accumulators (one record of a per-step series) -- sw_run_series.
+__global__ void k_snapshot(const Acc *acc, unsigned long long *dst, int words)
+{
+    const int k = threadIdx.x;
+    if (k < words) dst[k] = reinterpret_cast<const unsigned long long *>(acc)[k];
 }
 
 __global__ void k_philox_selftest(const uint32_t *ctr, const uint32_t *key, uint32_t *out, int count)

@@ -19,6 +19,14 @@ CONFIGS = {
 }
 
 
+# The remaining two of the paper's six programs: timed by
+# bench.py next to the five BASELINE configs, parity-tested at small sizes.
+EXTRA_CONFIGS = {
+    "X1": dict(dim=3, L=256, model=POTTS, q=3, T=1.8164, steps=500, desc="3D q=3 Potts L=256"),
+    "X2": dict(dim=2, L=2048, model=XY, q=0, T=0.8929, steps=500, desc="2D XY L=2048"),
+}
+
+
 def random_spins(model, N, q=0, seed=0):
     """Uniform random configuration (numpy PCG64, not the method's generator)."""
     rng = np.random.default_rng(seed)

@@ -348,3 +348,31 @@ def test_recording_does_not_change_the_trajectory():
     with pytest.raises(sw.SwError):
         a.bonds()
     assert b.bonds().shape == (64 ** 3,)
+
+
+@pytest.mark.parametrize("dim,L,model,q,T,n", [(2, 64, 0, 0, TC2, 300), (3, 32, 0, 0, T3, 60), (2, 96, 1, 3, TP3, 80),
+                                                  (3, 32, 1, 5, 1.4, 30), (3, 32, 2, 0, 2.2019, 20)])
+def test_observable_series_on_device(dim, L, model, q, T, n):
+    """sw_run_series (per-step E, M, M^2, M^4 kept on the device, one copy at the end)
+    against the oracle's per-step series: exact for Ising / Potts (integer sums), to fp32-sum accuracy
+    for XY; and identical to stepping with sw_observables after every step."""
+    sw, orc = _mods()
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=4)
+    h = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=4)
+    o = orc.Oracle(dim, L, model, q, 1.0 / T, 4)
+    sg = g.run_series(n)
+    so_ = o.run_series(n)
+    assert g.t == n
+    if model != 2:
+        assert np.array_equal(sg["E"], so_["E"]) and np.array_equal(sg["M"], so_["M"]) and np.array_equal(sg["M2"], so_["M2"])
+    else:
+        assert np.allclose(sg["E"], so_["E"], rtol=2e-6, atol=1e-2) and np.allclose(sg["M2"], so_["M2"], rtol=2e-5, atol=1e-2)
+    assert np.array_equal(sg["M4"], sg["M2"] ** 2)
+    for k in range(min(n, 10)):
+        h.step(1)
+        e, m, m2, m4 = h.observables()
+        if model != 2:
+            assert (e, m, m2, m4) == (sg["E"][k], sg["M"][k], sg["M2"][k], sg["M4"][k])
+        else:   # XY sums are fp64 atomics in arbitrary order: equal up to rounding
+            assert (e, m, m2, m4) == pytest.approx((sg["E"][k], sg["M"][k], sg["M2"][k], sg["M4"][k]), rel=1e-9)
+    assert np.array_equal(g.spins(), o.spins()) or model == 2
