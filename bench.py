@@ -278,6 +278,20 @@ def run_ours(args):
                        "bytes_per_site": kb,
                        "step": {"floor_bytes_per_site": floor_bytes_per_site(cfg["model"]), "achieved": step_gbs,
                                 "frac": step_gbs / peak}}
+    if rank == 0:
+        # north_star: "labelling-iteration counts" -- the union-find has no outer iteration, so what is
+        # reported is one counted step: unions attempted / linked / retried in the global merge, find
+        # hops there, and rounds of the root chase in the flip kernel
+        g.set_counting(True)
+        g.step(1)
+        st = g.label_stats()
+        g.set_counting(False)
+        act = max(st["active_border_bonds"], 1)
+        out["labelling"] = {"tile_face_bonds": st["border_bonds"], "active": st["active_border_bonds"],
+                            "unions_linked": st["unions_linked"], "cas_retries": st["union_retries"],
+                            "merge_hops_per_union": st["merge_find_hops"] / act, "merge_hops_max": st["merge_find_hops_max"],
+                            "chase_rounds_per_thread": st["chase_hops"] / (n_sites / 16), "chase_rounds_max": st["chase_hops_max"],
+                            "host_iterations": 0}
     if rank == 0 and not args.no_extras:
         # the paper's second row (Table 1): update + measurement of E and M every step,
         # through sw_run_series (per-step sums stay on the device)
