@@ -154,6 +154,11 @@ struct sw_ctx {
     void *workspace;
     uint8_t *bonds_mem;
     unsigned merge_blocks;
+    // CUDA graphs of 1 and GRAPH_STEPS consecutive steps (3 kernel nodes per step); built lazily for
+    // Ising / Potts, rebuilt when the bond-recording flag changes.  XY passes a new direction with
+    // every step and keeps plain launches.
+    cudaGraphExec_t graph1, graphK;
+    int graph_record;   // record_bonds state the graphs were built for (-1: none)
     bool own_workspace, own_stream;
     bool stepped;      // labels of a step are available
     bool bonds_valid;  // the last step recorded its bond bytes
@@ -347,7 +352,6 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     }
     p.L = (uint32_t)L; p.N = (uint32_t)c->N;
     p.k0 = (uint32_t)(seed & 0xffffffffu); p.k1 = (uint32_t)(seed >> 32);
-    p.t_lo = p.t_hi = 0;
     // PAPER.md:96 (garbled "p = 1 e^{2J/T}"): Ising p = 1 - exp(-2 beta); PAPER.md:152 + Eq. 2: Potts
     // p = 1 - exp(-beta).  The decision is the integer compare word < floor(p 2^32).
     const double prob = (model == SW_ISING) ? -std::expm1(-2.0 * beta) : -std::expm1(-beta);
@@ -356,6 +360,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     p.rx = 1.f; p.ry = 0.f; p.crefl = 0.f; p.m2beta = (float)(-2.0 * beta);
     p.counting = 0;
     c->force_phi = 0; c->forced_phi = 0.0; c->rx = c->ry = c->crefl = 0.f; c->sticky = 0;
+    c->graph1 = nullptr; c->graphK = nullptr; c->graph_record = -1;
     c->timing = 0; c->timed_steps = 0;
     for (int k = 0; k < 3; ++k) c->kernel_ms[k] = 0.0;
     for (int k = 0; k < 4; ++k) c->ev[k] = nullptr;
@@ -407,22 +412,76 @@ int sw_create_in(sw_ctx **out, int dim, int L, int model, int q, double beta, ui
     return create_common(out, dim, L, model, q, beta, seed, device_workspace, workspace_bytes, cuda_stream, true);
 }
 
+namespace {
+
+constexpr int GRAPH_STEPS = 16;
+
+// A graph of `steps` consecutive SW steps: k_bond_label -> k_merge -> k_flip, chained.  The kernels take
+// the step index from device memory, so the same graph serves every step.
+int build_graph(sw_ctx *c, int steps, cudaGraphExec_t *out)
+{
+    cudaGraph_t g = nullptr;
+    SW_CUDA(c, cudaGraphCreate(&g, 0));
+    Params p = c->p;
+    void *args[1] = {&p};
+    const dim3 grid = tile_grid(c);
+    cudaGraphNode_t prev = nullptr;
+    cudaError_t e = cudaSuccess;
+    for (int s = 0; s < steps && e == cudaSuccess; ++s) {
+        for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
+            cudaKernelNodeParams kp = {};
+            kp.kernelParams = args;
+            kp.extra = nullptr;
+            if (k == 0) { kp.func = (void *)c->ops.bond_label; kp.gridDim = grid; kp.blockDim = dim3(c->ops.nt); kp.sharedMemBytes = (unsigned)c->ops.smem_bond_label; }
+            if (k == 1) { kp.func = (void *)c->ops.merge; kp.gridDim = dim3(c->merge_blocks); kp.blockDim = dim3(256); kp.sharedMemBytes = 0; }
+            if (k == 2) { kp.func = (void *)c->ops.flip; kp.gridDim = grid; kp.blockDim = dim3(c->ops.nt); kp.sharedMemBytes = 0; }
+            cudaGraphNode_t node = nullptr;
+            e = cudaGraphAddKernelNode(&node, g, prev ? &prev : nullptr, prev ? 1 : 0, &kp);
+            prev = node;
+        }
+    }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(out, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) return cuda_fail(c, e, "building the step graph");
+    return SW_OK;
+}
+
+}  // namespace
+
 int sw_step(sw_ctx *c, int n)
 {
     int rc = check_ctx(c);
     if (rc) return rc;
     if (n < 0) return fail(SW_EINVAL, "n < 0");
     const dim3 grid = tile_grid(c);
+    if (c->model != SW_XY && !c->timing && !c->p.counting && n > 0 && !std::getenv("SW_B200_NO_GRAPH")) {
+        // launch-bound regime (small lattices): 3 launches per step cost more host time than the
+        // kernels take; replay pre-built graphs instead
+        if (c->graph_record != c->record_bonds) {
+            if (c->graph1) { cudaGraphExecDestroy(c->graph1); c->graph1 = nullptr; }
+            if (c->graphK) { cudaGraphExecDestroy(c->graphK); c->graphK = nullptr; }
+            c->p.bonds = c->record_bonds ? c->bonds_mem : nullptr;
+            rc = build_graph(c, 1, &c->graph1);
+            if (rc == SW_OK) rc = build_graph(c, GRAPH_STEPS, &c->graphK);
+            if (rc) return rc;
+            c->graph_record = c->record_bonds;
+        }
+        int left = n;
+        while (left >= GRAPH_STEPS) { SW_CUDA(c, cudaGraphLaunch(c->graphK, c->stream)); left -= GRAPH_STEPS; }
+        while (left > 0) { SW_CUDA(c, cudaGraphLaunch(c->graph1, c->stream)); --left; }
+        c->t += (uint64_t)n;
+        c->stepped = true; c->bonds_valid = c->record_bonds != 0;
+        c->M_fresh = true; c->E_fresh = false;
+        return SW_OK;
+    }
     for (int s = 0; s < n; ++s) {
         Params &p = c->p;
         p.bonds = c->record_bonds ? c->bonds_mem : nullptr;
-        p.t_lo = (uint32_t)(c->t & 0xffffffffu);
-        p.t_hi = (uint32_t)(c->t >> 32);
         if (c->model == SW_XY) {
             // PAPER.md:159 "randomly chosen" direction: phi uniform from one Philox word (domain 3),
             // r = (cos phi, sin phi) rounded to fp32; reflection constant c = (2 phi + pi) mod 2 pi.
             const double two_pi = 6.283185307179586476925286766559;
-            const uint4 w = philox4x32_10(0u, p.t_lo, p.t_hi, DOM_XYDIR, p.k0, p.k1);
+            const uint4 w = philox4x32_10(0u, (uint32_t)(c->t & 0xffffffffu), (uint32_t)(c->t >> 32), DOM_XYDIR, p.k0, p.k1);
             double phi = (double)w.x * (two_pi / 4294967296.0);
             if (c->force_phi) phi = c->forced_phi;
             p.rx = c->rx = (float)std::cos(phi);
@@ -532,6 +591,8 @@ int sw_destroy(sw_ctx *c)
 {
     if (!c) return SW_OK;
     cudaStreamSynchronize(c->stream);
+    if (c->graph1) cudaGraphExecDestroy(c->graph1);
+    if (c->graphK) cudaGraphExecDestroy(c->graphK);
     for (int k = 0; k < 4; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     if (c->own_workspace) cudaFree(c->workspace);
     if (c->own_stream) cudaStreamDestroy(c->stream);
@@ -561,6 +622,8 @@ int sw_set_spins(sw_ctx *c, const void *src, size_t bytes, uint64_t step)
     const size_t want = c->N * (c->model == SW_XY ? 4 : 1);
     if (!src || bytes != want) return fail(SW_EINVAL, "sw_set_spins: buffer must hold exactly N elements");
     SW_CUDA(c, cudaMemcpyAsync(c->p.spins, src, want, cudaMemcpyHostToDevice, c->stream));
+    const unsigned long long tdev = step;
+    SW_CUDA(c, cudaMemcpyAsync(&c->p.acc->t, &tdev, 8, cudaMemcpyHostToDevice, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
     c->t = step;
     c->stepped = false; c->bonds_valid = false; c->M_fresh = false; c->E_fresh = false;

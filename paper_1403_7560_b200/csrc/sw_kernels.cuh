@@ -56,6 +56,8 @@ struct Acc {
     unsigned long long nk[256];  // Potts: n_k
     unsigned long long stats[8]; // see sw_get_label_stats
     uint32_t npairs;             // length of the pair list of the current step
+    unsigned long long t;        // index of the step being executed: read by k_bond_label, advanced by
+                                 // k_flip, so a step's launches carry no per-step argument (CUDA graphs)
 };
 
 struct Params {
@@ -70,7 +72,6 @@ struct Params {
     uint32_t L, N;
     uint32_t ntx, nty, ntz, ntiles;
     uint32_t k0, k1;   // Philox key = (seed low, seed high)
-    uint32_t t_lo, t_hi;
     uint32_t P32;      // Ising/Potts: bond active iff word < P32
     int q;
     int db;            // draw bits in a label word: 1 (Ising, XY), ceil(log2 q) (Potts)
@@ -257,6 +258,8 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     const uint32_t tile_base = tile << G::LOG2NS;
     const int tid = threadIdx.x, lane = tid & 31;
     const uint32_t LL = L * L;
+    const unsigned long long t_step = p.acc->t;
+    const uint32_t t_lo = (uint32_t)t_step, t_hi = (uint32_t)(t_step >> 32);
 
     if (tid < G::NFW) face_s[tid] = 0u;
     if (tid == 0) { fpre_s[G::NFWP + 1] = 0u; fpre_s[G::NFWP + 2] = (uint32_t)G::LEFT_CAP; }
@@ -314,7 +317,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
         uint4 w[4];
         if (MODEL != ISING) {
 #pragma unroll
-            for (int s = 0; s < 4; ++s) w[s] = philox4x32_10(g + s, p.t_lo, p.t_hi, DOM_SITE, p.k0, p.k1);
+            for (int s = 0; s < 4; ++s) w[s] = philox4x32_10(g + s, t_lo, t_hi, DOM_SITE, p.k0, p.k1);
         }
         uint32_t bxn, byn, bzn = 0u, d;
         if (MODEL == XY) {
@@ -373,7 +376,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                 d = 0u;
                 uint32_t dmin = 0xffffffffu;
                 if (DIM == 2) {
-                    const uint4 c = philox4x32_10(g >> 2, p.t_lo, p.t_hi, DOM_PACK, p.k0, p.k1);
+                    const uint4 c = philox4x32_10(g >> 2, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
                     const uint32_t cw[4] = {c.x, c.y, c.z, c.w};
 #pragma unroll
                     for (int s = 3; s >= 0; --s) {
@@ -386,7 +389,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                 } else {
 #pragma unroll
                     for (int h = 1; h >= 0; --h) {
-                        const uint4 c = philox4x32_10((g >> 1) + h, p.t_lo, p.t_hi, DOM_PACK, p.k0, p.k1);
+                        const uint4 c = philox4x32_10((g >> 1) + h, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
                         const uint32_t lo[2] = {c.x, c.z}, hi[2] = {c.y, c.w};
 #pragma unroll
                         for (int u = 1; u >= 0; --u) {
@@ -410,16 +413,16 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                         const uint32_t i = g + s;
                         uint32_t e0, e1, e2 = ~0u;
                         if (DIM == 2) {
-                            const uint4 c = philox4x32_10(i >> 2, p.t_lo, p.t_hi, DOM_PACK, p.k0, p.k1);
+                            const uint4 c = philox4x32_10(i >> 2, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
                             const uint32_t w1 = (s == 0) ? c.x : (s == 1) ? c.y : (s == 2) ? c.z : c.w;
                             e0 = w1 & FM; e1 = (w1 >> F) & FM;
                         } else {
-                            const uint4 c = philox4x32_10(i >> 1, p.t_lo, p.t_hi, DOM_PACK, p.k0, p.k1);
+                            const uint4 c = philox4x32_10(i >> 1, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
                             const uint32_t l1 = (s & 1) ? c.z : c.x, h1 = (s & 1) ? c.w : c.y;
                             e0 = l1 & FM; e1 = __funnelshift_r(l1, h1, F) & FM; e2 = (h1 >> SH2) & FM;
                         }
                         if (e0 == Ptop || e1 == Ptop || e2 == Ptop) {
-                            const uint4 tw = philox4x32_10(i, p.t_lo, p.t_hi, DOM_TIE, p.k0, p.k1);
+                            const uint4 tw = philox4x32_10(i, t_lo, t_hi, DOM_TIE, p.k0, p.k1);
                             if (e0 == Ptop && (tw.x >> F) < Plow) rnx |= 1u << s;
                             if (e1 == Ptop && (tw.y >> F) < Plow) rny |= 1u << s;
                             if (DIM == 3 && e2 == Ptop && (tw.z >> F) < Plow) rnz |= 1u << s;
@@ -772,7 +775,10 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
         for (int k = tid; k < 256; k += NT) hist_s[k] = 0u;
         __syncthreads();
     }
-    if (tile == 0 && tid == 0) *p.npairs = 0u;  // k_merge of this step is done: empty list for the next one
+    if (tile == 0 && tid == 0) {
+        *p.npairs = 0u;   // k_merge of this step is done: empty list for the next one
+        p.acc->t += 1ull; // and the next k_bond_label works on the next step
+    }
     int m_loc = 0;
     uint32_t cnt_lo = 0u, cnt_hi = 0u;  // Potts, q <= 8: per-thread counts of states 0-3 / 4-7, one byte each
     unsigned chase_hops = 0;
