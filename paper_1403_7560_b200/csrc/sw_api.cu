@@ -26,7 +26,7 @@ int fail(int code, const std::string &msg)
 
 // One tile configuration = the tiled kernels instantiated for it.
 struct TileOps {
-    int tx, ty, tz, nt, nfw, log2ns;
+    int tx, ty, tz, nt, qpt, nfw, log2ns;
     size_t smem_bond_label;
     void (*bond_label)(const Params);
     void (*merge)(const Params);
@@ -35,14 +35,14 @@ struct TileOps {
     void (*tile_origin)(const Params);
 };
 
-template <int DIM, int MODEL, int TX, int TY, int TZ>
+template <int DIM, int MODEL, int TX, int TY, int TZ, int QPT = 4>
 TileOps make_ops()
 {
     using G = TileGeom<DIM, TX, TY, TZ>;
     constexpr int NS = G::NS;
-    constexpr int NT = NS / 16;  // 4 quads = 16 sites per thread
+    constexpr int NT = NS / (4 * QPT);  // QPT quads = 4 QPT sites per thread
     TileOps o;
-    o.tx = TX; o.ty = TY; o.tz = TZ; o.nt = NT; o.nfw = G::NFW; o.log2ns = G::LOG2NS;
+    o.tx = TX; o.ty = TY; o.tz = TZ; o.nt = NT; o.qpt = QPT; o.nfw = G::NFW; o.log2ns = G::LOG2NS;
     o.smem_bond_label = G::template smem_bond_label<MODEL>();
     o.bond_label = k_bond_label<DIM, MODEL, TX, TY, TZ, NT>;
     o.merge = k_merge<DIM, TX, TY, TZ>;
@@ -69,6 +69,25 @@ bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
 #undef SW_TILE2
 #undef SW_TILE3
     return false;
+}
+
+// Small lattices (fewer tiles than the GPU has room for): what counts is the critical path of one CTA,
+// so the smallest tile of the menu with ONE quad per thread (4x the threads for the same tile).
+template <int MODEL>
+bool pick_ops_small(int dim, TileOps &o)
+{
+    if (dim == 2) o = make_ops<2, MODEL, 32, 32, 1, 1>(); else o = make_ops<3, MODEL, 32, 8, 8, 1>();
+    return true;
+}
+
+bool pick_ops_small_model(int model, int dim, TileOps &o)
+{
+#ifdef SW_MENU_MIN
+    return false;
+#endif
+    if (model == SW_ISING) return pick_ops_small<ISING>(dim, o);
+    if (model == SW_POTTS) return pick_ops_small<POTTS>(dim, o);
+    return pick_ops_small<XY>(dim, o);
 }
 
 bool pick_ops_model(int model, int dim, int tx, int ty, int tz, TileOps &o)
@@ -325,6 +344,14 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     if (!ok) {
         tx = 32; ty = (dim == 2) ? 32 : 8; tz = (dim == 2) ? 1 : 8;
         pick_ops_model(model, dim, tx, ty, tz, c->ops);
+    }
+    if (!std::getenv("SW_B200_TILE")) {
+        // fewer default tiles than 2 per SM: latency variant (smallest tile, one quad per thread)
+        int sms = 148, dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const size_t ntiles_default = c->N / ((size_t)c->ops.tx * c->ops.ty * c->ops.tz);
+        if (ntiles_default < (size_t)2 * sms) pick_ops_small_model(model, dim, c->ops);
     }
     char *base = (char *)c->workspace;
     Params &p = c->p;
