@@ -376,3 +376,38 @@ def test_observable_series_on_device(dim, L, model, q, T, n):
         else:   # XY sums are fp64 atomics in arbitrary order: equal up to rounding
             assert (e, m, m2, m4) == pytest.approx((sg["E"][k], sg["M"][k], sg["M2"][k], sg["M4"][k]), rel=1e-9)
     assert np.array_equal(g.spins(), o.spins()) or model == 2
+
+
+@pytest.mark.parametrize("L,T,n", [(32, 2.269185, 200000), (64, 2.269185, 200000), (128, 2.269185, 60000), (64, 2.0, 60000), (64, 3.0, 60000)])
+def test_gpu_energy_against_exact_finite_torus(L, T, n):
+    """The CUDA path pinned to something other than the oracle: the long-run mean energy of the 2D
+    Ising chain against Kaufman's exact finite-torus value (tests/golden/kaufman_energy.txt, the
+    finite-L form of Onsager's result north_star names), and C/N = Var(E) / (N T^2) where the file has
+    it.  3 sigma with binned errors; a wrong bond probability, a missed wrap bond or a labelling
+    error shifts E/N by far more."""
+    import os
+    sw, _ = _mods()
+    from stats import binned_mean_err, golden_rows
+    rows = golden_rows(os.path.join(os.path.dirname(__file__), "golden", "kaufman_energy.txt"))
+    want = [r for r in rows if int(r[0]) == L and abs(float(r[1]) - T) < 1e-9][0]
+    e_exact, c_exact = float(want[2]), float(want[3])
+    N = L * L
+    errs = []
+    means = []
+    cs = []
+    for seed in (1, 2, 3, 4):            # the paper also uses four independent runs (PAPER.md:187)
+        g = sw.SwendsenWang(2, L, 0, 0, 1.0 / T, seed=seed)
+        g.step(1000)
+        s = g.run_series(n)
+        m, e = binned_mean_err(s["E"] / N, 64)
+        means.append(m)
+        errs.append(e)
+        cs.append(np.var(s["E"]) / (N * T * T))
+        g.close()
+    mean = float(np.mean(means))
+    err = float(np.sqrt(np.sum(np.square(errs))) / len(errs))
+    assert abs(mean - e_exact) <= 3.0 * err, f"E/N = {mean} +- {err}, exact {e_exact}"
+    assert err < 2e-3
+    if not math.isnan(c_exact):
+        c_mean, c_err = float(np.mean(cs)), float(np.std(cs, ddof=1) / np.sqrt(len(cs)))
+        assert abs(c_mean - c_exact) <= 4.0 * c_err + 0.02 * c_exact, f"C/N = {c_mean} +- {c_err}, exact {c_exact}"
