@@ -31,9 +31,6 @@ constexpr uint32_t FULL = 0xffffffffu;
 #ifndef SW_BL_THREADS_PER_SM
 #define SW_BL_THREADS_PER_SM 1536  // resident threads per SM k_bond_label is compiled for (register cap)
 #endif
-#ifndef SW_BL_INTERLEAVE
-#define SW_BL_INTERLEAVE 1
-#endif
 #ifndef SW_BL_ROUNDS
 #define SW_BL_ROUNDS 1  // uniform hook + flatten rounds before the general union-find loop
 #endif
@@ -149,24 +146,9 @@ __device__ __forceinline__ uint32_t spread4(uint32_t n) { return (n * 0x00204081
 // one, so the root of a finished tree is the minimum index of its set whatever the order in which
 // concurrent unions land.  Tile-local indices are monotone in the linear site index.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t find_s(volatile uint32_t *lab, uint32_t x)
-{
-    // path splitting: every node passed is re-pointed to its grandparent (plain stores of valid
-    // ancestors; a root is never written here, so the atomicMin hooks are not disturbed)
-    uint32_t p = lab[x];
-    while (p != x) {
-        const uint32_t gp = lab[p];
-        if (gp != p) lab[x] = gp;
-        x = p;
-        p = gp;
-    }
-    return x;
-}
-
 __device__ __forceinline__ void union_s(uint32_t *lab, uint32_t a, uint32_t b)
 {
     for (;;) {
-#if SW_BL_INTERLEAVE
         {   // both chains in one loop: trip count max(hops a, hops b) instead of the sum, two loads in flight
             volatile uint32_t *vl = lab;
             uint32_t pa = vl[a], pb = vl[b];
@@ -175,10 +157,6 @@ __device__ __forceinline__ void union_s(uint32_t *lab, uint32_t a, uint32_t b)
                 pa = vl[a]; pb = vl[b];
             }
         }
-#else
-        a = find_s(lab, a);
-        b = find_s(lab, b);
-#endif
         if (a == b) return;
         if (a < b) { const uint32_t t = a; a = b; b = t; }
         const uint32_t old = atomicMin(&lab[a], b);
