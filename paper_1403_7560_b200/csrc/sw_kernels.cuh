@@ -748,6 +748,8 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
     const int db = (MODEL == POTTS) ? p.db : 1;
     const uint32_t dm = (1u << db) - 1u;
     const uint32_t *__restrict__ lab = p.labels;
+    asm volatile("" : "+l"(lab));  // keep the base address in registers (else it is re-read from the constant bank per load)
+    const unsigned counting = p.counting ? 1u : 0u;
 
     if (MODEL == POTTS) {
         for (int k = tid; k < 256; k += NT) hist_s[k] = 0u;
@@ -771,18 +773,14 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
         uint32_t pw[4] = {w4.x, w4.y, w4.z, w4.w};
         uint32_t at[4] = {a0, a0 + 1u, a0 + 2u, a0 + 3u};
         for (;;) {
-            uint32_t moving = 0u;
-#pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                const uint32_t par = pw[s] >> db;
-                if (par != at[s]) {
-                    at[s] = par;
-                    pw[s] = __ldg(lab + par);
-                    moving = 1u;
-                }
-            }
-            if (!moving) break;
-            ++chase_hops;
+            const uint32_t q0 = pw[0] >> db, q1 = pw[1] >> db, q2 = pw[2] >> db, q3 = pw[3] >> db;
+            const bool m0 = q0 != at[0], m1 = q1 != at[1], m2 = q2 != at[2], m3 = q3 != at[3];
+            if (!(m0 | m1 | m2 | m3)) break;
+            if (m0) { at[0] = q0; pw[0] = __ldg(lab + q0); }
+            if (m1) { at[1] = q1; pw[1] = __ldg(lab + q1); }
+            if (m2) { at[2] = q2; pw[2] = __ldg(lab + q2); }
+            if (m3) { at[3] = q3; pw[3] = __ldg(lab + q3); }
+            chase_hops += counting;
         }
         __syncwarp();
 
