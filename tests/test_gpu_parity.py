@@ -61,6 +61,12 @@ def test_philox_device_known_answers():
     (3, 96, 0, 0, T3, 6),
     (3, 64, 1, 3, 1.8, 20),        # 3D Potts (one of the paper's six programs)
     (3, 32, 1, 20, 1.2, 20),       # q > 8: shared-memory histogram path
+    (2, 160, 0, 0, TC2, 12),       # tile sides that are not the default (L % 128 != 0, L % 64 != 0)
+    (2, 224, 1, 17, 0.9, 8),
+    (2, 2048, 0, 0, TC2, 3),       # default large-lattice tiling in 2D (128 x 64, four quads per thread)
+    (3, 160, 0, 0, T3, 3),         # default large-lattice tiling in 3D (32 x 16 x 16), L not a power of two
+    (3, 96, 1, 2, 1.1, 5),
+    (2, 64, 1, 255, 0.6, 10),      # largest q
 ])
 def test_full_trajectory_bit_exact(dim, L, model, q, T, steps):
     sw, orc = _mods()
@@ -223,7 +229,8 @@ def test_state_errors():
 # oracle is re-synchronised with the GPU's angles before every step (north_star: mismatch fraction
 # <= 1e-6 per step); where the bonds agree, labels, reflect decisions and angles must be identical.
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("dim,L,T,steps", [(3, 32, 2.2019, 12), (3, 64, 2.2019, 4), (2, 128, 0.9, 10), (3, 96, 1.5, 2)])
+@pytest.mark.parametrize("dim,L,T,steps", [(3, 32, 2.2019, 12), (3, 64, 2.2019, 4), (2, 128, 0.9, 10), (3, 96, 1.5, 2),
+                                           (2, 1056, 0.8929, 2), (3, 160, 2.2019, 2)])
 def test_xy_bond_mismatch_budget_and_exact_followup(dim, L, T, steps):
     sw, orc = _mods()
     g = sw.SwendsenWang(dim, L, 2, 0, 1.0 / T, seed=3, record_bonds=True)
