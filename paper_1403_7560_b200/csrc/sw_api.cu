@@ -110,8 +110,7 @@ void default_tile(int dim, int L, int model, int &tx, int &ty, int &tz)
         else if (L % 64 == 0) { tx = 64; ty = 64; }
         else { tx = 32; ty = 32; }
     } else {
-        tx = 32; ty = 16; tz = 16;
-        if (model == SW_XY) { ty = 8; tz = 8; }
+        tx = 32; ty = 16; tz = 16;  // also for XY (75 KB of shared memory per CTA: projections + labels)
     }
 }
 
