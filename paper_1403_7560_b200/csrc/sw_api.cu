@@ -106,8 +106,7 @@ void default_tile(int dim, int L, int model, int &tx, int &ty, int &tz)
 {
     if (dim == 2) {
         tz = 1;
-        if (L % 128 == 0) { tx = 128; ty = 64; }
-        else if (L % 64 == 0) { tx = 64; ty = 64; }
+        if (L % 64 == 0) { tx = 64; ty = 64; }   // measured on C2 / C3: 64x64 3 % ahead of 128x64
         else { tx = 32; ty = 32; }
     } else {
         tx = 32; ty = 16; tz = 16;  // also for XY (75 KB of shared memory per CTA: projections + labels)
