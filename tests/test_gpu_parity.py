@@ -418,3 +418,25 @@ def test_gpu_energy_against_exact_finite_torus(L, T, n):
     if not math.isnan(c_exact):
         c_mean, c_err = float(np.mean(cs)), float(np.std(cs, ddof=1) / np.sqrt(len(cs)))
         assert abs(c_mean - c_exact) <= 4.0 * c_err + 0.02 * c_exact, f"C/N = {c_mean} +- {c_err}, exact {c_exact}"
+
+
+def test_temperature_scan_moment_ratio_crossing():
+    """SURVEY.md 8(f)4, the paper's Figs. 1-2 in miniature: U(T) of the 3D Ising model for L = 32 and
+    L = 64 crosses near T_c = 4.51151 at U* ~ 1.6; U falls towards 1 below and rises
+    towards 3 above T_c, faster for the larger lattice.  Wide tolerances: corrections to scaling at
+    these sizes shift the crossing by ~0.01 in T."""
+    from paper_1403_7560_b200 import tscan
+    Ts = [4.40, 4.47, 4.50, 4.52, 4.55, 4.62]
+    r = tscan.scan(3, 0, [32, 64], Ts, n_discard=1500, n_measure=15000)
+    for L in (32, 64):
+        assert np.all(np.diff(r[L]["U"]) > 0), "U(T) must increase with T across the transition"
+        assert np.all(r[L]["U_err"] < 0.03)
+    assert r[64]["U"][0] < r[32]["U"][0] and r[64]["U"][-1] > r[32]["U"][-1]
+    cr = tscan.crossing(r, 32, 64)
+    assert cr is not None
+    Tx, Ux = cr
+    assert abs(Tx - 4.5115) < 0.03, f"crossing at T = {Tx}"
+    assert 1.45 < Ux < 1.75, f"U at the crossing = {Ux}"
+    # energy per site at T_c: literature value -0.9906 in the infinite lattice; finite L lies below
+    i = Ts.index(4.52)
+    assert -1.05 < r[64]["E"][i] < -0.95
