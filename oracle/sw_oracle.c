@@ -59,6 +59,8 @@ struct swo_ctx {
     int8_t *s_ising;   /* +-1          */
     uint8_t *s_potts;  /* 0..q-1       */
     float *s_xy;       /* angle theta  */
+    uint16_t *s_clock; /* clock state p, theta = 2 pi p / q */
+    int mirror;        /* clock: mirror index m of the last step */
     uint8_t *bond;     /* bit k = bond (i, i+e_k) active, last step */
     uint32_t *label;   /* min site index of the cluster, last step  */
     uint32_t *queue;   /* BFS work list */
@@ -109,6 +111,7 @@ static void init_spins(swo_ctx *o)
         draw(o, (uint32_t)i, 0, DOM_INIT, w);
         if (o->model == SWO_ISING) o->s_ising[i] = (w[0] >> 31) ? 1 : -1;
         else if (o->model == SWO_POTTS) o->s_potts[i] = (uint8_t)(((uint64_t)w[0] * (uint64_t)o->q) >> 32);
+        else if (o->model == SWO_CLOCK) o->s_clock[i] = (uint16_t)(((uint64_t)w[0] * (uint64_t)o->q) >> 32);
         else {
             float scale = (float)(TWO_PI / 16777216.0);
             o->s_xy[i] = (float)(w[0] >> 8) * scale;
@@ -120,25 +123,27 @@ swo_ctx *swo_create(int dim, int L, int model, int q, double beta, uint64_t seed
 {
     if (dim != 2 && dim != 3) return NULL;
     if (L < 3) return NULL; /* L = 2 would double every bond under periodic wrap */
-    if (model != SWO_ISING && model != SWO_POTTS && model != SWO_XY) return NULL;
+    if (model != SWO_ISING && model != SWO_POTTS && model != SWO_XY && model != SWO_CLOCK) return NULL;
     if (model == SWO_POTTS && (q < 2 || q > 255)) return NULL;
+    if (model == SWO_CLOCK && (q < 2 || q > 512)) return NULL; /* q <= 512 */
     if (!(beta >= 0.0) || !isfinite(beta)) return NULL;
     double Nd = pow((double)L, dim);
     if (Nd > 4294967295.0) return NULL;
     swo_ctx *o = (swo_ctx *)calloc(1, sizeof(*o));
     if (!o) return NULL;
-    o->dim = dim; o->L = L; o->model = model; o->q = (model == SWO_POTTS) ? q : 0;
+    o->dim = dim; o->L = L; o->model = model; o->q = (model == SWO_POTTS || model == SWO_CLOCK) ? q : 0;
     o->beta = beta; o->seed = seed; o->t = 0;
     o->N = 1;
     for (int a = 0; a < dim; ++a) o->N *= (size_t)L;
     if (model == SWO_ISING) o->s_ising = (int8_t *)malloc(o->N);
     if (model == SWO_POTTS) o->s_potts = (uint8_t *)malloc(o->N);
     if (model == SWO_XY) { o->s_xy = (float *)malloc(o->N * sizeof(float)); o->proj = (double *)malloc(o->N * sizeof(double)); }
+    if (model == SWO_CLOCK) { o->s_clock = (uint16_t *)malloc(o->N * sizeof(uint16_t)); o->proj = (double *)malloc(o->N * sizeof(double)); }
     o->bond = (uint8_t *)calloc(o->N, 1);
     o->label = (uint32_t *)malloc(o->N * sizeof(uint32_t));
     o->queue = (uint32_t *)malloc(o->N * sizeof(uint32_t));
-    if (!o->bond || !o->label || !o->queue || (!o->s_ising && !o->s_potts && !o->s_xy) ||
-        (model == SWO_XY && !o->proj)) { swo_destroy(o); return NULL; }
+    if (!o->bond || !o->label || !o->queue || (!o->s_ising && !o->s_potts && !o->s_xy && !o->s_clock) ||
+        ((model == SWO_XY || model == SWO_CLOCK) && !o->proj)) { swo_destroy(o); return NULL; }
     for (size_t i = 0; i < o->N; ++i) o->label[i] = (uint32_t)i;
     init_spins(o);
     return o;
@@ -147,7 +152,7 @@ swo_ctx *swo_create(int dim, int L, int model, int q, double beta, uint64_t seed
 void swo_destroy(swo_ctx *o)
 {
     if (!o) return;
-    free(o->s_ising); free(o->s_potts); free(o->s_xy); free(o->proj);
+    free(o->s_ising); free(o->s_potts); free(o->s_xy); free(o->s_clock); free(o->proj);
     free(o->bond); free(o->label); free(o->queue);
     free(o);
 }
@@ -231,6 +236,42 @@ static void make_bonds(swo_ctx *o)
             }
             o->bond[i] = b;
         }
+    } else if (o->model == SWO_CLOCK) {
+        /* q-state clock model (theta = 2 pi p / q; "The variable ispr, which
+         * is randomly chosen, specifies the direction for mirror projection").  Readings 23-25
+         * (DESIGN.md): the mirror index m = (word * q) >> 32 from the XYDIR call of the step; the
+         * mirror axis lies at angle pi m / q, so the reflection p -> (m - p) mod q maps clock states to
+         * clock states; the embedded Ising variable is the component along the normal of the axis,
+         * a(p) = sin(pi (2p - m) / q).  Written with k = (2p - m) mod 2q, u = k mod q:
+         * a = +sin(pi u / q) for k < q and -sin(pi u / q) for k >= q (zero for u = 0).  A bond between
+         * neighbours whose components have the same sign is active with
+         * p = 1 - exp(-2 beta a_i a_j), decided as word < floor(p 2^32) like Ising / Potts. */
+        uint32_t w[4];
+        const int q = o->q;
+        draw(o, 0, t, DOM_XYDIR, w);
+        const int m = (int)(((uint64_t)w[0] * (uint64_t)q) >> 32);
+        o->mirror = m;
+        for (size_t i = 0; i < o->N; ++i) {
+            int k = (2 * (int)o->s_clock[i] - m) % (2 * q);
+            if (k < 0) k += 2 * q;
+            int u = k % q;
+            double mag = sin((TWO_PI / 2.0) * (double)u / (double)q);
+            o->proj[i] = (u == 0) ? 0.0 : (k < q ? mag : -mag);
+        }
+        for (size_t i = 0; i < o->N; ++i) {
+            draw(o, (uint32_t)i, t, DOM_SITE, w);
+            uint8_t b = 0;
+            for (int k = 0; k < o->dim; ++k) {
+                size_t j = nbr_plus(o, i, k);
+                double ai = o->proj[i], aj = o->proj[j];
+                if ((ai > 0.0 && aj > 0.0) || (ai < 0.0 && aj < 0.0)) {
+                    double prod = fabs(ai) * fabs(aj);
+                    uint32_t P32 = threshold32(-expm1(-2.0 * o->beta * prod));
+                    if (w[k] < P32) { b |= (uint8_t)(1u << k); nact += 1.0; }
+                }
+            }
+            o->bond[i] = b;
+        }
     } else {
         /* XY: "we project vector spins to form Ising spin clusters" (Wolff's
          * embedding).  Reading 3: with a_i = r . s_i, a bond between neighbours whose projections
@@ -279,7 +320,7 @@ static void label_clusters(swo_ctx *o)
         double sum_a = 0.0;
         while (head < tail) {
             size_t i = o->queue[head++];
-            if (o->model == SWO_XY) sum_a += o->proj[i];
+            if (o->model == SWO_XY || o->model == SWO_CLOCK) sum_a += o->proj[i];
             for (int k = 0; k < o->dim; ++k) {
                 if (o->bond[i] & (1u << k)) {
                     size_t j = nbr_plus(o, i, k);
@@ -292,7 +333,7 @@ static void label_clusters(swo_ctx *o)
             }
         }
         nclus += 1.0;
-        snc2 += (o->model == SWO_XY) ? sum_a * sum_a : (double)tail * (double)tail;
+        snc2 += (o->model == SWO_XY || o->model == SWO_CLOCK) ? sum_a * sum_a : (double)tail * (double)tail;
     }
     o->n_clusters = nclus;
     o->sum_nc2 = snc2;
@@ -318,6 +359,15 @@ static void flip_clusters(swo_ctx *o)
             continue;
         }
         draw(o, o->label[i], t, DOM_SITE, w);
+        if (o->model == SWO_CLOCK) {
+            /* mirror projection of the whole cluster with probability 1/2: p -> (m - p) mod q */
+            if (w[3] >> 31) {
+                int pn = (o->mirror - (int)o->s_clock[i]) % o->q;
+                if (pn < 0) pn += o->q;
+                o->s_clock[i] = (uint16_t)pn;
+            }
+            continue;
+        }
         if (o->model == SWO_POTTS) o->s_potts[i] = (uint8_t)(((uint64_t)w[3] * (uint64_t)o->q) >> 32);
         else if (w[3] >> 31) {
             float th = o->crefl - o->s_xy[i];
@@ -344,7 +394,7 @@ int swo_step(swo_ctx *o, int n)
  * n[k] = number of spins in state k (Eq. 5). */
 int swo_counts(const swo_ctx *o, int64_t *E_int, int64_t *M_or_nk, int n)
 {
-    if (!o || o->model == SWO_XY) return -1;
+    if (!o || o->model == SWO_XY || o->model == SWO_CLOCK) return -1;
     int64_t E = 0;
     if (o->model == SWO_ISING) {
         int64_t M = 0;
@@ -381,6 +431,19 @@ void swo_observables(const swo_ctx *o, double *E, double *M, double *M2, double 
         for (int k = 0; k < o->q; ++k) s2 += (double)nk[k] * (double)nk[k];
         double Nd = (double)o->N;
         e = (double)Ei; m2 = ((double)o->q * s2 - Nd * Nd) / (double)(o->q - 1); m = sqrt(m2);
+    } else if (o->model == SWO_CLOCK) {
+        /* Eq. (3) with theta = 2 pi p / q, from the exact integer histograms (the paper's tables
+         * rule[] and fmy[]): E = -sum_d D[d] cos(2 pi d / q),
+         * M = | sum_p n[p] (cos, sin)(2 pi p / q) |, summed in increasing d and p. */
+        int64_t D[512], nn[512];
+        swo_clock_hist(o, D, nn, o->q);
+        double mx = 0.0, my = 0.0;
+        for (int d = 0; d < o->q; ++d) e -= (double)D[d] * cos(TWO_PI * (double)d / (double)o->q);
+        for (int pp = 0; pp < o->q; ++pp) {
+            mx += (double)nn[pp] * cos(TWO_PI * (double)pp / (double)o->q);
+            my += (double)nn[pp] * sin(TWO_PI * (double)pp / (double)o->q);
+        }
+        m2 = mx * mx + my * my; m = sqrt(m2);
     } else {
         double mx = 0.0, my = 0.0;
         for (size_t i = 0; i < o->N; ++i) {
@@ -396,13 +459,40 @@ void swo_observables(const swo_ctx *o, double *E, double *M, double *M2, double 
     if (M4) *M4 = m2 * m2;
 }
 
+int swo_clock_hist(const swo_ctx *o, int64_t *D, int64_t *n, int q)
+{
+    if (!o || o->model != SWO_CLOCK || q != o->q) return -1;
+    for (int k = 0; k < q; ++k) { if (D) D[k] = 0; if (n) n[k] = 0; }
+    for (size_t i = 0; i < o->N; ++i) {
+        int pi_ = (int)o->s_clock[i];
+        if (n) n[pi_] += 1;
+        for (int k = 0; k < o->dim && D; ++k) {
+            int d = (pi_ - (int)o->s_clock[nbr_plus(o, i, k)]) % q;
+            if (d < 0) d += q;
+            D[d] += 1;
+        }
+    }
+    return 0;
+}
+
+int swo_get_clock_mirror(const swo_ctx *o, int *m)
+{
+    if (!o || o->model != SWO_CLOCK) return -1;
+    if (m) *m = o->mirror;
+    return 0;
+}
+
 size_t swo_num_sites(const swo_ctx *o) { return o ? o->N : 0; }
 uint64_t swo_step_index(const swo_ctx *o) { return o ? o->t : 0; }
 
-static size_t spin_bytes(const swo_ctx *o) { return o->model == SWO_XY ? o->N * sizeof(float) : o->N; }
+static size_t spin_bytes(const swo_ctx *o)
+{
+    return o->model == SWO_XY ? o->N * sizeof(float) : o->model == SWO_CLOCK ? o->N * sizeof(uint16_t) : o->N;
+}
 static void *spin_ptr(const swo_ctx *o)
 {
-    return o->model == SWO_ISING ? (void *)o->s_ising : o->model == SWO_POTTS ? (void *)o->s_potts : (void *)o->s_xy;
+    return o->model == SWO_ISING ? (void *)o->s_ising : o->model == SWO_POTTS ? (void *)o->s_potts
+         : o->model == SWO_CLOCK ? (void *)o->s_clock : (void *)o->s_xy;
 }
 
 int swo_get_spins(const swo_ctx *o, void *dst, size_t bytes)

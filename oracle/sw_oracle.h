@@ -27,13 +27,13 @@ extern "C" {
 
 typedef struct swo_ctx swo_ctx;
 
-enum { SWO_ISING = 0, SWO_POTTS = 1, SWO_XY = 2 };
+enum { SWO_ISING = 0, SWO_POTTS = 1, SWO_XY = 2, SWO_CLOCK = 3 };
 
 /* Philox4x32-10, exposed so that the tests can pin it to the known-answer vectors. */
 void swo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 
-/* dim in {2,3}; L >= 3 (any L, not only multiples of 32); model as enum; q used by Potts only
- * (2..255); beta = J/T with J = 1; returns NULL on invalid arguments or out of memory.
+/* dim in {2,3}; L >= 3 (any L, not only multiples of 32); model as enum; q = number of Potts states
+ * (2..255) or clock states (2..512), ignored otherwise; beta = J/T with J = 1; returns NULL on invalid arguments or out of memory.
  * The start configuration is the seeded random start (S3), step counter t = 0. */
 swo_ctx *swo_create(int dim, int L, int model, int q, double beta, uint64_t seed);
 void swo_destroy(swo_ctx *o);
@@ -48,7 +48,8 @@ void swo_observables(const swo_ctx *o, double *E, double *M, double *M2, double 
  * Potts: E = number of unequal nearest-neighbour pairs, M_or_nk[k] = n[k], k < q). */
 int swo_counts(const swo_ctx *o, int64_t *E_int, int64_t *M_or_nk, int n);
 
-/* State access.  Spins are int8 (Ising, +-1), uint8 (Potts, 0..q-1) or float (XY angle). */
+/* State access.  Spins are int8 (Ising, +-1), uint8 (Potts, 0..q-1), float (XY angle) or uint16
+ * (clock state 0..q-1). */
 size_t swo_num_sites(const swo_ctx *o);
 uint64_t swo_step_index(const swo_ctx *o);
 int swo_get_spins(const swo_ctx *o, void *dst, size_t bytes);
@@ -57,6 +58,11 @@ int swo_get_bonds(const swo_ctx *o, uint8_t *dst, size_t bytes);    /* bonds of 
 int swo_get_labels(const swo_ctx *o, uint32_t *dst, size_t bytes);  /* labels of the LAST step */
 /* XY: direction (r_x, r_y as fp32) and reflection constant c of the LAST step. */
 int swo_get_xy_dir(const swo_ctx *o, float *rx, float *ry, float *c);
+/* Clock model: exact integer histograms of the current configuration: D[d] = number of nearest-
+ * neighbour pairs (i, i + e_k) with (p_i - p_j) mod q = d, n[p] = number of sites in state p. */
+int swo_clock_hist(const swo_ctx *o, int64_t *D, int64_t *n, int q);
+/* Clock model: mirror index m (the paper's ispr) of the LAST step. */
+int swo_get_clock_mirror(const swo_ctx *o, int *m);
 /* XY test hook (special case R2 in DESIGN.md): force phi for every following step. */
 int swo_force_xy_phi(swo_ctx *o, int enable, double phi);
 

@@ -10,7 +10,7 @@ import numpy as np
 
 from . import build as _build
 
-ISING, POTTS, XY = 0, 1, 2
+ISING, POTTS, XY, CLOCK = 0, 1, 2, 3
 
 _lib = None
 
@@ -37,6 +37,8 @@ def lib():
         L.swo_get_xy_dir.argtypes = [C.c_void_p] + [C.POINTER(C.c_float)] * 3
         L.swo_force_xy_phi.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.swo_run_series.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 6
+        L.swo_clock_hist.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.swo_get_clock_mirror.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
         L.swo_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
         _lib = L
     return _lib
@@ -50,7 +52,7 @@ def philox4x32_10(ctr, key):
     return [int(x) for x in o]
 
 
-_SPIN_DTYPE = {ISING: np.int8, POTTS: np.uint8, XY: np.float32}
+_SPIN_DTYPE = {ISING: np.int8, POTTS: np.uint8, XY: np.float32, CLOCK: np.uint16}
 
 
 class Oracle:
@@ -112,6 +114,17 @@ class Oracle:
         a = np.empty(self.N, dtype=np.uint32)
         assert lib().swo_get_labels(self._h, a.ctypes.data, a.nbytes) == 0
         return a
+
+    def clock_hist(self):
+        D = np.zeros(self.q, dtype=np.int64)
+        n = np.zeros(self.q, dtype=np.int64)
+        assert lib().swo_clock_hist(self._h, D.ctypes.data, n.ctypes.data, self.q) == 0
+        return D, n
+
+    def clock_mirror(self):
+        m = C.c_int()
+        assert lib().swo_get_clock_mirror(self._h, C.byref(m)) == 0
+        return int(m.value)
 
     def xy_dir(self):
         v = [C.c_float() for _ in range(3)]

@@ -140,3 +140,21 @@ def kaufman_energy_per_site(L, T, dps=None):
     d2 = mp.diff(f, K, 2)
     N = L * L
     return float(-d1 / N), float(K * K * d2 / N)
+
+
+def exact_clock(dim, L, q, T):
+    """Boltzmann averages of the q-state clock model (Eq. 3 with theta = 2 pi p / q, PAPER.md:84-88,
+    J = 1) by enumeration of all q^N states: <E>, <E^2>, <M^2> with M = |sum_i (cos, sin) theta_i|."""
+    s = enumerate_spin_states(dim, L, q).astype(np.int64)
+    bonds = lattice_bonds(dim, L)
+    ang = 2.0 * np.pi / q
+    E = np.zeros(s.shape[0], dtype=np.float64)
+    for (i, j) in bonds:
+        E -= np.cos(ang * (s[:, i] - s[:, j]))
+    mx = np.cos(ang * s).sum(axis=1)
+    my = np.sin(ang * s).sum(axis=1)
+    w = np.exp(-(E - E.min()) / T)
+    Z = w.sum()
+    avg = lambda x: float((w * x).sum() / Z)
+    M2 = mx * mx + my * my
+    return {"N": L ** dim, "n_bonds": len(bonds), "E": avg(E), "E2": avg(E * E), "M2": avg(M2), "M4": avg(M2 * M2)}
