@@ -48,19 +48,19 @@ def dist_env():
 
 
 def spin_bytes(model):
-    return 4 if model == 2 else 1
+    return 4 if model == 2 else (2 if model == 3 else 1)
 
 
 def floor_bytes_per_site(model):
     """spins read once and written once, a 4-byte label written before and
     read after the grid-wide merge; XY re-reads theta in the flip."""
-    return 20 if model == 2 else 10
+    return 20 if model == 2 else (14 if model == 3 else 10)   # clock: uint16 states, re-read in the flip
 
 
 def kernel_bytes_per_site(model):
     """Algorithmic bytes per site of each kernel."""
     sp = spin_bytes(model)
-    return {"k_bond_label": sp + 4, "k_merge": 0, "k_flip": 4 + sp + (sp if model == 2 else 0)}
+    return {"k_bond_label": sp + 4, "k_merge": 0, "k_flip": 4 + sp + (sp if model in (2, 3) else 0)}
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the one
@@ -118,7 +118,7 @@ def load_peak():
 # ---------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------
-DEFAULT_BURN_IN = {"C1": 200, "C2": 200, "C3": 200, "C4": 150, "C5": 100, "X1": 100, "X2": 100}
+DEFAULT_BURN_IN = {"C1": 200, "C2": 200, "C3": 200, "C4": 150, "C5": 100, "X1": 100, "X2": 100, "X3": 100}
 L2_BYTES = 126 * 2 ** 20
 
 
@@ -254,7 +254,7 @@ def run_ours(args):
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
         "ms_per_step": ms_all, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32" if cfg["model"] == 2 else ("u8" if cfg["model"] == 1 else "int8"), "data": "synthetic",
+        "dtype": {0: "int8", 1: "u8", 2: "f32", 3: "u16"}[cfg["model"]], "data": "synthetic",
         "config": {"workload": f"{args.config}: {cfg['desc']} periodic, T={cfg['T']:.6f}, Philox seed {args.seed}"
                                f" (+rank), seeded random start thermalised by {burn} untimed SW steps",
                    "sites": n_sites, "burn_in_steps": burn,

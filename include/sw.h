@@ -49,7 +49,7 @@ extern "C" {
 
 typedef struct sw_ctx sw_ctx;
 
-enum { SW_ISING = 0, SW_POTTS = 1, SW_XY = 2 };
+enum { SW_ISING = 0, SW_POTTS = 1, SW_XY = 2, SW_CLOCK = 3 };
 enum { SW_OK = 0, SW_EINVAL = -1, SW_ENOMEM = -2, SW_ECUDA = -3, SW_ESTATE = -4 };
 
 /* ---- the four calls of the hot path ------------------------------------------------------- */
@@ -57,8 +57,9 @@ enum { SW_OK = 0, SW_EINVAL = -1, SW_ENOMEM = -2, SW_ECUDA = -3, SW_ESTATE = -4 
 /* Create a context for a dim-dimensional (2 or 3) periodic lattice of linear size L with a seeded
  * random start configuration (device_function_spinset) and step counter t = 0.
  *   L      multiple of 32 ("nx ... multiple of 32"), L >= 32, L^dim <= 2^31;
- *   model  SW_ISING | SW_POTTS | SW_XY;  q: number of Potts states, 2..255 (ignored otherwise),
- *          with L^dim * 2^ceil(log2 q) <= 2^32 (a label word holds a site address and a state);
+ *   model  SW_ISING | SW_POTTS | SW_XY | SW_CLOCK;  q: number of Potts states, 2..255, with
+ *          L^dim * 2^ceil(log2 q) <= 2^32 (a label word holds a site address and a state), or number
+ *          of clock states, 2..512; ignored otherwise;
  *   beta   J/T with J = 1, finite, >= 0;  seed: Philox key.
  * Device memory comes from cudaMalloc and the context owns a new non-blocking stream.
  * On failure *out = NULL. */
@@ -82,6 +83,7 @@ int sw_step(sw_ctx *c, int n);
  *   Potts: E = number of unequal nearest-neighbour pairs (Eq. 2), M2 = (q sum_k n_k^2 - N^2)/(q-1)
  *          (Eq. 5), M = sqrt(M2), M4 = M2^2.
  *   XY:    E = -sum_<ij> cos(theta_i - theta_j) (Eq. 3), M = |sum_i (cos, sin)|, M2, M4 likewise.
+ *   Clock: as XY with theta = 2 pi p / q, from exact integer histograms.
  * Averages, the specific heat and the moment ratio (Eq. 6) are the caller's job.  Spins injected
  * with sw_set_spins must lie in the model's range (Ising +-1, Potts 0..q-1): the sums are taken
  * from byte-equality counts. */
@@ -106,7 +108,7 @@ size_t sw_num_sites(const sw_ctx *c);
 uint64_t sw_step_index(const sw_ctx *c);
 
 /* Copy the configuration to / from a HOST buffer of exactly N elements: int8 (Ising, +-1),
- * uint8 (Potts, 0..q-1) or float32 (XY angle in [0, 2 pi]).  sw_set_spins also sets the step
+ * uint8 (Potts, 0..q-1), float32 (XY angle in [0, 2 pi]) or uint16 (clock state 0..q-1).  sw_set_spins also sets the step
  * counter (state = (spins, seed, t), because the generator is counter-based).  Both synchronise.
  * Values outside the model's range are not checked. */
 int sw_get_spins(sw_ctx *c, void *host_dst, size_t bytes);
@@ -128,6 +130,15 @@ int sw_get_labels(sw_ctx *c, uint32_t *host_dst, size_t bytes);
  * host_M_or_nk[0] = sum s_i (n >= 1).  Potts: *host_E = #unequal pairs, host_M_or_nk[k] = n_k for
  * k < min(n, q).  SW_EINVAL for XY. */
 int sw_get_counts(sw_ctx *c, int64_t *host_E, int64_t *host_M_or_nk, int n);
+
+/* Clock model (SW_CLOCK: the q-state clock discretisation of XY the paper's program runs, PAPER.md:88,
+ * 159, 210; spins are uint16 states p = 0..q-1, theta = 2 pi p / q).  Exact integer histograms of the
+ * current configuration: host_D[d] = number of nearest-neighbour pairs (i, i + e_k) with
+ * (p_i - p_j) mod q = d, host_n[p] = number of sites in state p (q entries each, either may be NULL);
+ * and the mirror index m (the paper's ispr) of the LAST step: the step reflects a cluster as
+ * p -> (m - p) mod q. */
+int sw_get_clock_hist(sw_ctx *c, int64_t *host_D, int64_t *host_n, int q);
+int sw_get_clock_mirror(sw_ctx *c, int *host_m);
 
 /* XY: direction r = (rx, ry) and reflection constant c = (2 phi + pi) mod 2 pi of the LAST step. */
 int sw_get_xy_dir(sw_ctx *c, float *host_rx, float *host_ry, float *host_c);

@@ -3,4 +3,4 @@
 The product is libsw_b200.so (csrc/, C ABI in include/sw.h); this package builds it in-tree and
 exposes the thin ctypes binding.  No CPU fallback exists: without the built CUDA library or a
 CUDA device the calls raise."""
-from .binding import ISING, POTTS, XY, SwendsenWang, SwError, lib, philox_selftest  # noqa: F401
+from .binding import CLOCK, ISING, POTTS, XY, SwendsenWang, SwError, lib, philox_selftest  # noqa: F401

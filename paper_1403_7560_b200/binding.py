@@ -11,10 +11,10 @@ import numpy as np
 
 from . import build as _build
 
-ISING, POTTS, XY = 0, 1, 2
+ISING, POTTS, XY, CLOCK = 0, 1, 2, 3
 SW_OK, SW_EINVAL, SW_ENOMEM, SW_ECUDA, SW_ESTATE = 0, -1, -2, -3, -4
 
-_SPIN_DTYPE = {ISING: np.int8, POTTS: np.uint8, XY: np.float32}
+_SPIN_DTYPE = {ISING: np.int8, POTTS: np.uint8, XY: np.float32, CLOCK: np.uint16}
 
 _lib = None
 
@@ -52,6 +52,8 @@ def lib():
     L.sw_get_bonds.argtypes = [vp, vp, sz]
     L.sw_get_labels.argtypes = [vp, vp, sz]
     L.sw_get_counts.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), i32]
+    L.sw_get_clock_hist.argtypes = [vp, vp, vp, i32]
+    L.sw_get_clock_mirror.argtypes = [vp, C.POINTER(i32)]
     L.sw_get_xy_dir.argtypes = [vp] + [C.POINTER(C.c_float)] * 3
     L.sw_force_xy_phi.argtypes = [vp, i32, dbl]
     L.sw_set_counting.argtypes = [vp, i32]
@@ -176,6 +178,17 @@ class SwendsenWang:
         a = np.empty(self.N, dtype=np.uint32)
         _check(lib().sw_get_labels(self._h, a.ctypes.data, a.nbytes))
         return a
+
+    def clock_hist(self):
+        D = np.zeros(self.q, dtype=np.int64)
+        n = np.zeros(self.q, dtype=np.int64)
+        _check(lib().sw_get_clock_hist(self._h, D.ctypes.data, n.ctypes.data, self.q))
+        return D, n
+
+    def clock_mirror(self):
+        m = C.c_int()
+        _check(lib().sw_get_clock_mirror(self._h, C.byref(m)))
+        return int(m.value)
 
     def xy_dir(self):
         v = [C.c_float() for _ in range(3)]

@@ -87,6 +87,7 @@ bool pick_ops_small_model(int model, int dim, TileOps &o)
 #endif
     if (model == SW_ISING) return pick_ops_small<ISING>(dim, o);
     if (model == SW_POTTS) return pick_ops_small<POTTS>(dim, o);
+    if (model == SW_CLOCK) return pick_ops_small<CLOCK>(dim, o);
     return pick_ops_small<XY>(dim, o);
 }
 
@@ -98,6 +99,7 @@ bool pick_ops_model(int model, int dim, int tx, int ty, int tz, TileOps &o)
 #endif
     if (model == SW_ISING) return pick_ops<ISING>(dim, tx, ty, tz, o);
     if (model == SW_POTTS) return pick_ops<POTTS>(dim, tx, ty, tz, o);
+    if (model == SW_CLOCK) return pick_ops<CLOCK>(dim, tx, ty, tz, o);
     return pick_ops<XY>(dim, tx, ty, tz, o);
 }
 
@@ -127,8 +129,9 @@ bool valid_args(int dim, int L, int model, int q, double beta, bool check_beta)
 {
     if (dim != 2 && dim != 3) return false;
     if (L < 32 || L % 32 != 0) return false;
-    if (model != SW_ISING && model != SW_POTTS && model != SW_XY) return false;
+    if (model != SW_ISING && model != SW_POTTS && model != SW_XY && model != SW_CLOCK) return false;
     if (model == SW_POTTS && (q < 2 || q > 255)) return false;
+    if (model == SW_CLOCK && (q < 2 || q > 512)) return false;  // q <= 512
     if (check_beta && !(std::isfinite(beta) && beta >= 0.0)) return false;
     double n = std::pow((double)L, dim);
     if (n > 2147483648.0) return false;
@@ -137,15 +140,17 @@ bool valid_args(int dim, int L, int model, int q, double beta, bool check_beta)
     return true;
 }
 
-struct Layout { size_t spins, bonds, labels, pairs, origin, acc, total; };
+struct Layout { size_t spins, bonds, labels, pairs, origin, table, acc, total; };
 
-Layout layout(int dim, int L, int model)
+size_t spin_bytes(int model) { return model == SW_XY ? 4 : (model == SW_CLOCK ? 2 : 1); }
+
+Layout layout(int dim, int L, int model, int q)
 {
     size_t N = 1;
     for (int a = 0; a < dim; ++a) N *= (size_t)L;
     Layout l;
     size_t off = 0;
-    l.spins = off; off += align256(N * (model == SW_XY ? 4 : 1));
+    l.spins = off; off += align256(N * spin_bytes(model));
     l.bonds = off; off += align256(N);
     l.labels = off; off += align256(N * 4);
     // pair list: one (i, j) address pair per bond through a tile face, sized for the tile of the menu
@@ -153,6 +158,7 @@ Layout layout(int dim, int L, int model)
     // tile origins (smallest tile: 1024 sites)
     l.pairs = off; off += align256((dim == 3 ? N / 32 * 9 : N / 16) * 8);
     l.origin = off; off += align256((N / 1024) * 4);
+    l.table = off; off += align256(model == SW_CLOCK ? (size_t)q * q * 4 : 0);  // clock: bond thresholds
     l.acc = off; off += align256(sizeof(Acc));
     l.total = off;
     return l;
@@ -185,6 +191,7 @@ struct sw_ctx {
     int force_phi;
     double forced_phi;
     float rx, ry, crefl;
+    int mirror;
     int sticky;
     int timing;            // per-kernel event timing mode
     cudaEvent_t ev[4];
@@ -248,6 +255,12 @@ void launch_measure_dm(sw_ctx *c, bool with_m)
 
 void launch_measure(sw_ctx *c, bool with_m)
 {
+    if (c->model == SW_CLOCK) {
+        const unsigned g = (unsigned)(c->N / 256);
+        if (c->dim == 2) k_measure_clock<2><<<g, 256, 0, c->stream>>>(c->p);
+        else k_measure_clock<3><<<g, 256, 0, c->stream>>>(c->p);
+        return;
+    }
     if (c->dim == 2) {
         if (c->model == SW_ISING) launch_measure_dm<2, ISING>(c, with_m);
         else if (c->model == SW_POTTS) launch_measure_dm<2, POTTS>(c, with_m);
@@ -263,7 +276,7 @@ void launch_measure(sw_ctx *c, bool with_m)
 int refresh_observables(sw_ctx *c)
 {
     if (c->E_fresh && c->M_fresh) return SW_OK;
-    const bool with_m = !c->M_fresh;
+    const bool with_m = !c->M_fresh || c->model == SW_CLOCK;  // clock: both histograms in one pass
     // E_int and E_xy are the first 16 bytes of Acc; the magnetisation sums follow.
     const size_t clear = with_m ? offsetof(Acc, stats) : offsetof(Acc, M_int);
     SW_CUDA(c, cudaMemsetAsync(c->p.acc, 0, clear, c->stream));
@@ -274,10 +287,27 @@ int refresh_observables(sw_ctx *c)
 }
 
 // Extensive observables from the accumulator head (E_int, E_xy, M_int, mx, my, n_k[q]).
-void sums_to_observables(const sw_ctx *c, const unsigned long long *w, double &e, double &m, double &m2)
+void sums_to_observables(const sw_ctx *c, const unsigned long long *w, const unsigned long long *nk,
+                         const unsigned long long *dk, double &e, double &m, double &m2)
 {
     double dv[5];
     std::memcpy(dv, w, sizeof(dv));
+    if (c->model == SW_CLOCK) {
+        // Eq. (3) with theta = 2 pi p / q from the exact histograms (the paper's tables rule[] and
+        // fmy[]), summed in increasing d and p
+        const double two_pi = 6.283185307179586476925286766559;
+        const int q = c->q;
+        double mx = 0.0, my = 0.0;
+        e = 0.0;
+        for (int d = 0; d < q; ++d) e -= (double)(long long)dk[d] * std::cos(two_pi * (double)d / (double)q);
+        for (int pp = 0; pp < q; ++pp) {
+            mx += (double)(long long)nk[pp] * std::cos(two_pi * (double)pp / (double)q);
+            my += (double)(long long)nk[pp] * std::sin(two_pi * (double)pp / (double)q);
+        }
+        m2 = mx * mx + my * my;
+        m = std::sqrt(m2);
+        return;
+    }
     if (c->model == SW_ISING) {
         e = (double)(long long)w[0];
         m = (double)(long long)w[2];
@@ -285,7 +315,7 @@ void sums_to_observables(const sw_ctx *c, const unsigned long long *w, double &e
     } else if (c->model == SW_POTTS) {
         // Eq. (5): M^2 = (q sum_k n_k^2 - N^2) / (q - 1)
         double s2 = 0.0;
-        for (int k = 0; k < c->q; ++k) s2 += (double)w[5 + k] * (double)w[5 + k];
+        for (int k = 0; k < c->q; ++k) s2 += (double)nk[k] * (double)nk[k];
         const double Nd = (double)c->N;
         e = (double)(long long)w[0];
         m2 = ((double)c->q * s2 - Nd * Nd) / (double)(c->q - 1);
@@ -304,7 +334,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     *out = nullptr;
     if (!valid_args(dim, L, model, q, beta, true))
         return fail(SW_EINVAL, "invalid arguments (dim 2|3, L multiple of 32 with L^dim <= 2^31 and L^dim 2^ceil(log2 q) <= 2^32, model, 2<=q<=255, beta>=0)");
-    const Layout lay = layout(dim, L, model);
+    const Layout lay = layout(dim, L, model, q);
     if (external) {
         if (!workspace || workspace_bytes < lay.total || ((uintptr_t)workspace & 255u))
             return fail(SW_EINVAL, "device workspace missing, too small or not 256-byte aligned");
@@ -317,7 +347,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     }
     sw_ctx *c = new (std::nothrow) sw_ctx();
     if (!c) return fail(SW_ENOMEM, "host allocation failed");
-    c->dim = dim; c->L = L; c->model = model; c->q = (model == SW_POTTS) ? q : 0;
+    c->dim = dim; c->L = L; c->model = model; c->q = (model == SW_POTTS || model == SW_CLOCK) ? q : 0;
     c->beta = beta; c->seed = seed; c->t = 0;
     c->N = lay.total ? 1 : 0;
     for (int a = 0; a < dim; ++a) c->N *= (size_t)L;
@@ -383,6 +413,8 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     p.P32 = threshold32(prob);
     p.q = c->q;
     p.rx = 1.f; p.ry = 0.f; p.crefl = 0.f; p.m2beta = (float)(-2.0 * beta);
+    p.clock_T = (const uint32_t *)(base + lay.table);
+    p.mirror = 0; c->mirror = 0;
     p.counting = 0;
     c->force_phi = 0; c->forced_phi = 0.0; c->rx = c->ry = c->crefl = 0.f; c->sticky = 0;
     c->graph1 = nullptr; c->graphK = nullptr; c->graph_record = -1;
@@ -404,8 +436,23 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     if (e != cudaSuccess) return bail(e, "k_tile_origin launch");
     e = cudaMemsetAsync(p.acc, 0, sizeof(Acc), c->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync");
+    if (model == SW_CLOCK) {
+        // clock model, reading 24: component along the mirror normal |a(u)| = sin(pi u / q), u = 1..q-1;
+        // bond threshold T[u_i q + u_j] = floor((1 - exp(-2 beta a_i a_j)) 2^32), in double on the host
+        const double two_pi = 6.283185307179586476925286766559;
+        std::vector<double> mag((size_t)q, 0.0);
+        for (int u = 0; u < q; ++u) mag[u] = std::sin((two_pi / 2.0) * (double)u / (double)q);
+        std::vector<uint32_t> tab((size_t)q * q, 0u);
+        for (int ui = 1; ui < q; ++ui)
+            for (int uj = 1; uj < q; ++uj)
+                tab[(size_t)ui * q + uj] = threshold32(-std::expm1(-2.0 * beta * (mag[ui] * mag[uj])));
+        e = cudaMemcpyAsync((void *)p.clock_T, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);  // tab goes out of scope
+        if (e != cudaSuccess) return bail(e, "clock threshold table");
+    }
     if (model == SW_ISING) launch_init<ISING>(c);
     else if (model == SW_POTTS) launch_init<POTTS>(c);
+    else if (model == SW_CLOCK) launch_init<CLOCK>(c);
     else launch_init<XY>(c);
     e = cudaGetLastError();
     if (e != cudaSuccess) return bail(e, "k_init launch");
@@ -423,7 +470,7 @@ const char *sw_last_error(void) { return g_err.c_str(); }
 size_t sw_workspace_bytes(int dim, int L, int model, int q)
 {
     if (!valid_args(dim, L, model, q, 0.0, false)) return 0;
-    return layout(dim, L, model).total;
+    return layout(dim, L, model, q).total;
 }
 
 int sw_create(sw_ctx **out, int dim, int L, int model, int q, double beta, uint64_t seed)
@@ -479,7 +526,7 @@ int sw_step(sw_ctx *c, int n)
     if (rc) return rc;
     if (n < 0) return fail(SW_EINVAL, "n < 0");
     const dim3 grid = tile_grid(c);
-    if (c->model != SW_XY && !c->timing && !c->p.counting && n > 0 && !std::getenv("SW_B200_NO_GRAPH")) {
+    if (c->model != SW_XY && c->model != SW_CLOCK && !c->timing && !c->p.counting && n > 0 && !std::getenv("SW_B200_NO_GRAPH")) {
         // launch-bound regime (small lattices): 3 launches per step cost more host time than the
         // kernels take; replay pre-built graphs instead
         if (c->graph_record != c->record_bonds) {
@@ -513,6 +560,12 @@ int sw_step(sw_ctx *c, int n)
             p.ry = c->ry = (float)std::sin(phi);
             p.crefl = c->crefl = (float)std::fmod(2.0 * phi + two_pi / 2.0, two_pi);
         }
+        if (c->model == SW_CLOCK) {
+            // "The variable ispr, which is randomly chosen, specifies the direction for
+            // mirror projection": m = (word q) >> 32 from the XYDIR call of the step (reading 23)
+            const uint4 w = philox4x32_10(0u, (uint32_t)(c->t & 0xffffffffu), (uint32_t)(c->t >> 32), DOM_XYDIR, p.k0, p.k1);
+            p.mirror = c->mirror = (int)(((unsigned long long)w.x * (unsigned long long)c->q) >> 32);
+        }
         if (p.counting) {
             SW_CUDA(c, cudaMemsetAsync(p.acc->stats, 0, sizeof(p.acc->stats), c->stream));
             const unsigned long long examined = (unsigned long long)c->N / c->ops.tx + c->N / c->ops.ty +
@@ -540,7 +593,7 @@ int sw_step(sw_ctx *c, int n)
     if (n > 0) {
         SW_CUDA(c, cudaGetLastError());
         c->stepped = true; c->bonds_valid = c->record_bonds != 0;
-        c->M_fresh = (c->model != SW_XY);  // XY: the vector magnetisation is summed on request
+        c->M_fresh = (c->model != SW_XY && c->model != SW_CLOCK);  // XY, clock: the magnetisation is summed on request
         c->E_fresh = false;
     }
     return SW_OK;
@@ -556,7 +609,7 @@ int sw_observables(sw_ctx *c, double *E, double *M, double *M2, double *M4)
     SW_CUDA(c, cudaMemcpyAsync(&h, c->p.acc, offsetof(Acc, stats), cudaMemcpyDeviceToHost, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
     double e, m, m2;
-    sums_to_observables(c, (const unsigned long long *)&h, e, m, m2);
+    sums_to_observables(c, (const unsigned long long *)&h, h.nk, h.dk, e, m, m2);
     if (E) *E = e;
     if (M) *M = m;
     if (M2) *M2 = m2;
@@ -571,7 +624,8 @@ int sw_run_series(sw_ctx *c, int n, double *E, double *M, double *M2, double *M4
     if (n < 0) return fail(SW_EINVAL, "n < 0");
     if (n == 0) return SW_OK;
     // per step one record of 5 + q 64-bit words = the head of Acc (E_int, E_xy, M_int, mx, my, n_k)
-    const int words = 5 + c->q;
+    const int w1 = 5 + c->q, w2 = (c->model == SW_CLOCK) ? c->q : 0, words = w1 + w2;
+    const int off2 = (int)(offsetof(Acc, dk) / 8);
     unsigned long long *dser = nullptr;
     cudaError_t e = cudaMalloc(&dser, (size_t)n * words * 8);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SW_ENOMEM, "sw_run_series: cudaMalloc of the series buffer failed"); }
@@ -579,7 +633,7 @@ int sw_run_series(sw_ctx *c, int n, double *E, double *M, double *M2, double *M4
         rc = sw_step(c, 1);
         if (rc == SW_OK) rc = refresh_observables(c);
         if (rc == SW_OK) {
-            k_snapshot<<<1, 288, 0, c->stream>>>(c->p.acc, dser + (size_t)s * words, words);
+            k_snapshot<<<1, 1024, 0, c->stream>>>(c->p.acc, dser + (size_t)s * words, w1, off2, w2);
             if (cudaGetLastError() != cudaSuccess) rc = fail(SW_ECUDA, "k_snapshot launch");
         }
     }
@@ -596,11 +650,10 @@ int sw_run_series(sw_ctx *c, int n, double *E, double *M, double *M2, double *M4
         cudaStreamSynchronize(c->stream);
     }
     if (rc == SW_OK) {
-        std::vector<unsigned long long> rec(5 + 256, 0ull);
         for (int s = 0; s < n; ++s) {
-            std::memcpy(rec.data(), hser + (size_t)s * words, (size_t)words * 8);
+            const unsigned long long *rec = hser + (size_t)s * words;
             double ev, m, m2;
-            sums_to_observables(c, rec.data(), ev, m, m2);
+            sums_to_observables(c, rec, rec + 5, rec + w1, ev, m, m2);
             if (E) E[s] = ev;
             if (M) M[s] = m;
             if (M2) M2[s] = m2;
@@ -633,7 +686,7 @@ int sw_get_spins(sw_ctx *c, void *dst, size_t bytes)
 {
     int rc = check_ctx(c);
     if (rc) return rc;
-    const size_t want = c->N * (c->model == SW_XY ? 4 : 1);
+    const size_t want = c->N * spin_bytes(c->model);
     if (!dst || bytes != want) return fail(SW_EINVAL, "sw_get_spins: buffer must hold exactly N elements");
     SW_CUDA(c, cudaMemcpyAsync(dst, c->p.spins, want, cudaMemcpyDeviceToHost, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -644,7 +697,7 @@ int sw_set_spins(sw_ctx *c, const void *src, size_t bytes, uint64_t step)
 {
     int rc = check_ctx(c);
     if (rc) return rc;
-    const size_t want = c->N * (c->model == SW_XY ? 4 : 1);
+    const size_t want = c->N * spin_bytes(c->model);
     if (!src || bytes != want) return fail(SW_EINVAL, "sw_set_spins: buffer must hold exactly N elements");
     SW_CUDA(c, cudaMemcpyAsync(c->p.spins, src, want, cudaMemcpyHostToDevice, c->stream));
     const unsigned long long tdev = step;
@@ -694,6 +747,7 @@ int sw_get_counts(sw_ctx *c, int64_t *E, int64_t *M_or_nk, int n)
     int rc = check_ctx(c);
     if (rc) return rc;
     if (c->model == SW_XY) return fail(SW_EINVAL, "sw_get_counts: integer sums are not defined for XY");
+    if (c->model == SW_CLOCK) return fail(SW_EINVAL, "sw_get_counts: use sw_get_clock_hist for the clock model");
     rc = refresh_observables(c);
     if (rc) return rc;
     Acc h;
@@ -704,6 +758,33 @@ int sw_get_counts(sw_ctx *c, int64_t *E, int64_t *M_or_nk, int n)
         if (c->model == SW_ISING) { if (n >= 1) M_or_nk[0] = (int64_t)h.M_int; }
         else for (int k = 0; k < n && k < c->q; ++k) M_or_nk[k] = (int64_t)h.nk[k];
     }
+    return SW_OK;
+}
+
+int sw_get_clock_hist(sw_ctx *c, int64_t *D, int64_t *n, int q)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (c->model != SW_CLOCK || q != c->q) return fail(SW_EINVAL, "sw_get_clock_hist: not a clock context, or q differs");
+    rc = refresh_observables(c);
+    if (rc) return rc;
+    Acc h;
+    SW_CUDA(c, cudaMemcpyAsync(&h, c->p.acc, offsetof(Acc, stats), cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < q; ++k) {
+        if (D) D[k] = (int64_t)h.dk[k];
+        if (n) n[k] = (int64_t)h.nk[k];
+    }
+    return SW_OK;
+}
+
+int sw_get_clock_mirror(sw_ctx *c, int *m)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (c->model != SW_CLOCK) return fail(SW_EINVAL, "not a clock context");
+    if (!c->stepped) return fail(SW_ESTATE, "no step since create / sw_set_spins");
+    if (m) *m = c->mirror;
     return SW_OK;
 }
 

@@ -25,7 +25,7 @@
 
 namespace swk {
 
-enum { ISING = 0, POTTS = 1, XY = 2 };
+enum { ISING = 0, POTTS = 1, XY = 2, CLOCK = 3 };
 constexpr uint32_t DOM_SITE = 0u, DOM_PACK = 1u, DOM_INIT = 2u, DOM_XYDIR = 3u, DOM_TIE = 4u;
 constexpr uint32_t FULL = 0xffffffffu;
 #ifndef SW_BL_THREADS_PER_SM
@@ -50,7 +50,8 @@ struct Acc {
     double E_xy;                 // XY: -sum cos(theta_i - theta_j)
     unsigned long long M_int;    // Ising: sum s_i (two's complement)
     double mx, my;               // XY: sum cos, sum sin
-    unsigned long long nk[256];  // Potts: n_k
+    unsigned long long nk[512];  // Potts: n_k (q <= 255); clock: number of sites in state p (q <= 512)
+    unsigned long long dk[512];  // clock: number of nearest-neighbour pairs with (p_i - p_j) mod q = d
     unsigned long long stats[8]; // see sw_get_label_stats
     uint32_t npairs;             // length of the pair list of the current step
     unsigned long long t;        // index of the step being executed: read by k_bond_label, advanced by
@@ -73,6 +74,8 @@ struct Params {
     int q;
     int db;            // draw bits in a label word: 1 (Ising, XY), ceil(log2 q) (Potts)
     float rx, ry, crefl, m2beta;  // XY: direction, reflection constant, -2 beta
+    const uint32_t *clock_T;      // clock: q x q bond thresholds T[u_i q + u_j] (see k_bond_label)
+    int mirror;                   // clock: mirror index m of the step (the paper's ispr)
     int counting;
 };
 
@@ -190,6 +193,7 @@ __global__ void __launch_bounds__(256) k_init(const Params p)
     const uint32_t w = philox4x32_10(i, 0u, 0u, DOM_INIT, p.k0, p.k1).x;
     if (MODEL == ISING) ((int8_t *)p.spins)[i] = (w >> 31) ? 1 : -1;
     else if (MODEL == POTTS) ((uint8_t *)p.spins)[i] = (uint8_t)(((unsigned long long)w * (unsigned)p.q) >> 32);
+    else if (MODEL == CLOCK) ((uint16_t *)p.spins)[i] = (uint16_t)(((unsigned long long)w * (unsigned)p.q) >> 32);
     else ((float *)p.spins)[i] = (float)(w >> 8) * (float)(6.283185307179586476925286766559 / 16777216.0);
 }
 
@@ -324,6 +328,43 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                     const float pz = av[s] * azv[s];
                     if (pz > 0.f && (float)(w[s].z >> 8) * scale < -expm1f(p.m2beta * pz)) bzn |= 1u << s;
                 }
+            }
+            d = (w[0].w >> 31) | ((w[1].w >> 31) << 1) | ((w[2].w >> 31) << 2) | ((w[3].w >> 31) << 3);
+        } else if (MODEL == CLOCK) {
+            // q-state clock model (readings 23-25): state p, mirror index m.
+            // k = (2p - m) mod 2q, u = k mod q: the component along the mirror normal is
+            // +sin(pi u / q) for k < q, -sin(pi u / q) for k >= q, zero for u = 0.  A bond between
+            // neighbours of the same non-zero sign is active iff word < T[u_i q + u_j], the table
+            // floor((1 - exp(-2 beta sin sin)) 2^32) built once on the host.
+            const uint16_t *sp = (const uint16_t *)p.spins;
+            const int q = p.q, m = p.mirror;
+            auto cls = [&](uint32_t pp) -> uint32_t {  // u | sign class << 16 (1: positive, 2: negative, 0: zero)
+                int k = 2 * (int)pp - m;
+                if (k < 0) k += 2 * q;
+                const int u = k >= q ? k - q : k;
+                return (uint32_t)u | (u == 0 ? 0u : (k >= q ? 2u : 1u) << 16);
+            };
+            const uint2 own2 = *reinterpret_cast<const uint2 *>(sp + g);
+            const uint2 up2 = *reinterpret_cast<const uint2 *>(sp + ((gy + 1 == L) ? g - L * (L - 1) : g + L));
+            uint32_t nbq = __shfl_down_sync(FULL, own2.x, 1) & 0xffffu;
+            if (rowend) nbq = sp[(gx + 4 == L) ? g + 4 - L : g + 4];
+            const uint32_t c0[5] = {cls(own2.x & 0xffffu), cls(own2.x >> 16), cls(own2.y & 0xffffu), cls(own2.y >> 16), cls(nbq)};
+            const uint32_t cy[4] = {cls(up2.x & 0xffffu), cls(up2.x >> 16), cls(up2.y & 0xffffu), cls(up2.y >> 16)};
+            uint32_t cz[4] = {0u, 0u, 0u, 0u};
+            if (DIM == 3) {
+                const uint2 fr2 = *reinterpret_cast<const uint2 *>(sp + ((gz + 1 == L) ? g - LL * (L - 1) : g + LL));
+                cz[0] = cls(fr2.x & 0xffffu); cz[1] = cls(fr2.x >> 16); cz[2] = cls(fr2.y & 0xffffu); cz[3] = cls(fr2.y >> 16);
+            }
+            auto bond = [&](uint32_t a, uint32_t b, uint32_t word) -> uint32_t {
+                if (((a & b) >> 16) == 0u) return 0u;  // different sign, or one component is zero
+                return word < __ldg(p.clock_T + (a & 0xffffu) * (uint32_t)q + (b & 0xffffu)) ? 1u : 0u;
+            };
+            bxn = byn = 0u;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                bxn |= bond(c0[s], c0[s + 1], w[s].x) << s;
+                byn |= bond(c0[s], cy[s], w[s].y) << s;
+                if (DIM == 3) bzn |= bond(c0[s], cz[s], w[s].z) << s;
             }
             d = (w[0].w >> 31) | ((w[1].w >> 31) << 1) | ((w[2].w >> 31) << 2) | ((w[3].w >> 31) << 3);
         } else {
@@ -807,6 +848,21 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
                 atomicAdd(&hist_s[d2], 1u);
                 atomicAdd(&hist_s[d3], 1u);
             }
+        } else if (MODEL == CLOCK) {
+            // PAPER.md:159 mirror projection of the cluster: p -> (m - p) mod q
+            if ((pw[0] | pw[1] | pw[2] | pw[3]) & 1u) {
+                uint2 v = *reinterpret_cast<uint2 *>((uint16_t *)p.spins + g);
+                uint32_t st[4] = {v.x & 0xffffu, v.x >> 16, v.y & 0xffffu, v.y >> 16};
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    if (pw[s] & 1u) {
+                        int n = p.mirror - (int)st[s];
+                        if (n < 0) n += p.q;
+                        st[s] = (uint32_t)n;
+                    }
+                }
+                *reinterpret_cast<uint2 *>((uint16_t *)p.spins + g) = make_uint2(st[0] | (st[1] << 16), st[2] | (st[3] << 16));
+            }
         } else {
             // PAPER.md:159 mirror projection: theta' = c - theta, wrapped into [0, 2 pi]
             if ((pw[0] | pw[1] | pw[2] | pw[3]) & 1u) {
@@ -1014,11 +1070,51 @@ __global__ void __launch_bounds__(256) k_measure4(const Params p)
     }
 }
 
-// k_snapshot: copy the head of the accumulators (one record of a per-step series) -- sw_run_series.
-__global__ void k_snapshot(const Acc *acc, unsigned long long *dst, int words)
+// ------------------------------------------------------------------------------------------------
+// k_measure_clock: the exact integer histograms of the clock model -- n[p] (sites per state, the
+// paper's fmy[] table gives M from it) and D[d] (nearest-neighbour pairs per state difference, the
+// paper's rule[] table gives E from it).  One site per thread, shared histograms.
+// ------------------------------------------------------------------------------------------------
+template <int DIM>
+__global__ void __launch_bounds__(256) k_measure_clock(const Params p)
 {
-    const int k = threadIdx.x;
-    if (k < words) dst[k] = reinterpret_cast<const unsigned long long *>(acc)[k];
+    __shared__ uint32_t n_s[512], d_s[512];
+    const int tid = threadIdx.x;
+    for (int k = tid; k < 512; k += 256) { n_s[k] = 0u; d_s[k] = 0u; }
+    __syncthreads();
+    const uint32_t i = blockIdx.x * 256u + tid;  // N is a multiple of 1024
+    const uint32_t L = p.L;
+    uint32_t x, y, z;
+    decode(p, i, x, y, z);
+    const uint16_t *s = (const uint16_t *)p.spins;
+    const int q = p.q, v = s[i];
+    atomicAdd(&n_s[v], 1u);
+    const uint32_t jx = (x + 1 == L) ? i - (L - 1) : i + 1;
+    const uint32_t jy = (y + 1 == L) ? i - L * (L - 1) : i + L;
+    int dx = v - (int)s[jx], dy = v - (int)s[jy];
+    if (dx < 0) dx += q;
+    if (dy < 0) dy += q;
+    atomicAdd(&d_s[dx], 1u);
+    atomicAdd(&d_s[dy], 1u);
+    if (DIM == 3) {
+        const uint32_t jz = (z + 1 == L) ? i - L * L * (L - 1) : i + L * L;
+        int dz = v - (int)s[jz];
+        if (dz < 0) dz += q;
+        atomicAdd(&d_s[dz], 1u);
+    }
+    __syncthreads();
+    for (int k = tid; k < q; k += 256) {
+        if (n_s[k]) atomicAdd(&p.acc->nk[k], (unsigned long long)n_s[k]);
+        if (d_s[k]) atomicAdd(&p.acc->dk[k], (unsigned long long)d_s[k]);
+    }
+}
+
+// k_snapshot: copy the head of the accumulators (one record of a per-step series) -- sw_run_series:
+// w1 words from the start, then w2 words from word offset off2 (the clock model's D[d]).
+__global__ void __launch_bounds__(1024) k_snapshot(const Acc *acc, unsigned long long *dst, int w1, int off2, int w2)
+{
+    const unsigned long long *src = reinterpret_cast<const unsigned long long *>(acc);
+    for (int k = threadIdx.x; k < w1 + w2; k += 1024) dst[k] = k < w1 ? src[k] : src[off2 + (k - w1)];
 }
 
 __global__ void k_philox_selftest(const uint32_t *ctr, const uint32_t *key, uint32_t *out, int count)

@@ -6,7 +6,7 @@ import math
 
 import numpy as np
 
-ISING, POTTS, XY = 0, 1, 2
+ISING, POTTS, XY, CLOCK = 0, 1, 2, 3
 
 # BASELINE.json configs: name -> (dim, L, model, q, T, steps)
 CONFIGS = {
@@ -24,6 +24,9 @@ CONFIGS = {
 EXTRA_CONFIGS = {
     "X1": dict(dim=3, L=256, model=POTTS, q=3, T=1.8164, steps=500, desc="3D q=3 Potts L=256"),
     "X2": dict(dim=2, L=2048, model=XY, q=0, T=0.8929, steps=500, desc="2D XY L=2048"),
+    # the model the paper's XY program and its Table 2 actually use: the 512-state clock model
+    # (PAPER.md:159, 210), at the configuration of C5
+    "X3": dict(dim=3, L=256, model=CLOCK, q=512, T=2.2019, steps=500, desc="3D 512-state clock L=256"),
 }
 
 
@@ -34,6 +37,8 @@ def random_spins(model, N, q=0, seed=0):
         return (2 * rng.integers(0, 2, size=N, dtype=np.int8) - 1).astype(np.int8)
     if model == POTTS:
         return rng.integers(0, q, size=N, dtype=np.uint8)
+    if model == CLOCK:
+        return rng.integers(0, q, size=N).astype(np.uint16)
     return (rng.random(N, dtype=np.float32) * np.float32(2.0 * math.pi)).astype(np.float32)
 
 
@@ -43,6 +48,8 @@ def aligned_spins(model, N, value=None):
         return np.full(N, 1 if value is None else value, dtype=np.int8)
     if model == POTTS:
         return np.full(N, 0 if value is None else value, dtype=np.uint8)
+    if model == CLOCK:
+        return np.full(N, 1 if value is None else value, dtype=np.uint16)
     return np.full(N, 0.5 if value is None else value, dtype=np.float32)
 
 
@@ -56,6 +63,8 @@ def striped_spins(model, dim, L, width, q=2):
         return (2 * (band % 2) - 1).astype(np.int8)
     if model == POTTS:
         return (band % q).astype(np.uint8)
+    if model == CLOCK:
+        return (band % q).astype(np.uint16)
     return ((band % 2) * np.float32(math.pi)).astype(np.float32)
 
 
@@ -67,6 +76,8 @@ def domain_spins(model, dim, L, block, q=2, seed=0):
         vals = (2 * rng.integers(0, 2, size=nb ** dim) - 1).astype(np.int8)
     elif model == POTTS:
         vals = rng.integers(0, q, size=nb ** dim).astype(np.uint8)
+    elif model == CLOCK:
+        vals = rng.integers(0, q, size=nb ** dim).astype(np.uint16)
     else:
         vals = (rng.random(nb ** dim) * 2.0 * math.pi).astype(np.float32)
     idx = np.arange(L ** dim, dtype=np.int64)

@@ -440,3 +440,70 @@ def test_temperature_scan_moment_ratio_crossing():
     # energy per site at T_c: literature value -0.9906 in the infinite lattice; finite L lies below
     i = Ts.index(4.52)
     assert -1.05 < r[64]["E"][i] < -0.95
+
+
+# ------------------------------------------------------------------------------------------------
+# q-state clock model (the model the paper's XY program runs):
+# integer states, so everything is bit-exact against the oracle.
+# ------------------------------------------------------------------------------------------------
+def _compare_clock_step(g, o, tag):
+    assert g.clock_mirror() == o.clock_mirror(), f"{tag}: mirror index differs"
+    bg, bo = g.bonds(), o.bonds()
+    assert np.array_equal(bg, bo), f"{tag}: bonds differ at {np.flatnonzero(bg != bo)[:8]}"
+    assert np.array_equal(g.labels(), o.labels()), f"{tag}: labels differ"
+    assert np.array_equal(g.spins(), o.spins()), f"{tag}: states differ"
+    Dg, ng = g.clock_hist()
+    Do, no = o.clock_hist()
+    assert np.array_equal(Dg, Do) and np.array_equal(ng, no), f"{tag}: histograms differ"
+    assert g.observables() == pytest.approx(o.observables(), rel=1e-13, abs=1e-9)
+
+
+@pytest.mark.parametrize("dim,L,q,T,steps", [
+    (2, 64, 8, 0.9, 200), (2, 32, 4, 1.13, 100), (2, 96, 5, 0.8, 30), (2, 256, 512, 0.9, 20), (2, 2048, 16, 0.9, 2),
+    (3, 32, 512, 2.2019, 40), (3, 64, 6, 2.0, 12), (3, 96, 2, 3.0, 4), (3, 160, 512, 2.2019, 2),
+])
+def test_clock_full_trajectory_bit_exact(dim, L, q, T, steps):
+    sw, orc = _mods()
+    g = sw.SwendsenWang(dim, L, 3, q, 1.0 / T, seed=2, record_bonds=True)
+    o = orc.Oracle(dim, L, 3, q, 1.0 / T, 2)
+    assert np.array_equal(g.spins(), o.spins()), "seeded start differs"
+    for t in range(steps):
+        g.step(1)
+        o.step(1)
+        _compare_clock_step(g, o, f"clock dim{dim} L{L} q{q} t={t}")
+    g.close()
+
+
+def test_clock_injected_states_series_and_full_size():
+    sw, orc = _mods()
+    from paper_1403_7560_b200 import inputs
+    # structured states at low temperature: long clusters across tiles and the wrap
+    g = sw.SwendsenWang(3, 64, 3, 12, 1.0 / 1.2, seed=5, record_bonds=True)
+    o = orc.Oracle(3, 64, 3, 12, 1.0 / 1.2, 5)
+    for k, s in enumerate([inputs.striped_spins(3, 3, 64, 5, 12), inputs.domain_spins(3, 3, 64, 24, 12, seed=2),
+                           inputs.aligned_spins(3, 64 ** 3)]):
+        g.set_spins(s, 100 * k)
+        o.set_spins(s, 100 * k)
+        for t in range(2):
+            g.step(1)
+            o.step(1)
+            _compare_clock_step(g, o, f"state {k} t={t}")
+    g.close()
+    # per-step series kept on the device
+    g = sw.SwendsenWang(2, 64, 3, 8, 1.0 / 0.9, seed=3)
+    o = orc.Oracle(2, 64, 3, 8, 1.0 / 0.9, 3)
+    sg, so_ = g.run_series(100), o.run_series(100)
+    assert np.allclose(sg["E"], so_["E"], rtol=1e-13, atol=1e-9) and np.allclose(sg["M2"], so_["M2"], rtol=1e-12, atol=1e-8)
+    g.close()
+    # the paper's size: 512-state clock model on 256^3 at the configuration of C5, one sampled step
+    g = sw.SwendsenWang(3, 256, 3, 512, 1.0 / 2.2019, seed=1)
+    o = orc.Oracle(3, 256, 3, 512, 1.0 / 2.2019, 1)
+    g.step(30)
+    o.set_spins(g.spins(), g.t)
+    g.step(1)
+    o.step(1)
+    assert g.clock_mirror() == o.clock_mirror()
+    assert np.array_equal(g.labels(), o.labels()) and np.array_equal(g.spins(), o.spins())
+    Dg, ng = g.clock_hist()
+    Do, no = o.clock_hist()
+    assert np.array_equal(Dg, Do) and np.array_equal(ng, no)
