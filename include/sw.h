@@ -126,6 +126,12 @@ int sw_set_record_bonds(sw_ctx *c, int enable);
 int sw_get_bonds(sw_ctx *c, uint8_t *host_dst, size_t bytes);
 int sw_get_labels(sw_ctx *c, uint32_t *host_dst, size_t bytes);
 
+/* Cluster statistics of the LAST executed step's labelling (on request; scratch device memory of
+ * N x 4 bytes for the call): number of clusters and sum over clusters of the squared cluster size.
+ * For Ising and Potts <sum_c n_c^2> = <M^2> (the improved estimator of the Fortuin-Kasteleyn
+ * representation; Potts with Eq. (5)'s normalisation).  Either pointer may be NULL. */
+int sw_get_cluster_stats(sw_ctx *c, uint64_t *host_n_clusters, uint64_t *host_sum_nc2);
+
 /* Exact integer sums of the current configuration.  Ising: *host_E = -sum s_i s_j,
  * host_M_or_nk[0] = sum s_i (n >= 1).  Potts: *host_E = #unequal pairs, host_M_or_nk[k] = n_k for
  * k < min(n, q).  SW_EINVAL for XY. */

@@ -51,6 +51,7 @@ def lib():
     L.sw_set_record_bonds.argtypes = [vp, i32]
     L.sw_get_bonds.argtypes = [vp, vp, sz]
     L.sw_get_labels.argtypes = [vp, vp, sz]
+    L.sw_get_cluster_stats.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
     L.sw_get_counts.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), i32]
     L.sw_get_clock_hist.argtypes = [vp, vp, vp, i32]
     L.sw_get_clock_mirror.argtypes = [vp, C.POINTER(i32)]
@@ -146,6 +147,12 @@ class SwendsenWang:
         out = {k: np.empty(n, dtype=np.float64) for k in ("E", "M", "M2", "M4")}
         _check(lib().sw_run_series(self._h, int(n), *[out[k].ctypes.data for k in ("E", "M", "M2", "M4")]))
         return out
+
+    def cluster_stats(self):
+        """(number of clusters, sum of squared cluster sizes) of the last step's labelling."""
+        a, b = C.c_uint64(), C.c_uint64()
+        _check(lib().sw_get_cluster_stats(self._h, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
 
     def counts(self):
         n = self.q if self.model == POTTS else 1

@@ -742,6 +742,32 @@ int sw_get_labels(sw_ctx *c, uint32_t *dst, size_t bytes)
     return SW_OK;
 }
 
+int sw_get_cluster_stats(sw_ctx *c, uint64_t *n_clusters, uint64_t *sum_nc2)
+{
+    int rc = check_ctx(c);
+    if (rc) return rc;
+    if (!c->stepped) return fail(SW_ESTATE, "no step since create / sw_set_spins");
+    uint32_t *sizes = nullptr;
+    cudaError_t e = cudaMalloc(&sizes, c->N * 4 + 16);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SW_ENOMEM, "sw_get_cluster_stats: cudaMalloc of the size counters failed"); }
+    unsigned long long *out = (unsigned long long *)(sizes + c->N);
+    unsigned long long h[2] = {0ull, 0ull};
+    e = cudaMemsetAsync(sizes, 0, c->N * 4 + 16, c->stream);
+    if (e == cudaSuccess) {
+        const unsigned g = (unsigned)(c->N / 256);
+        k_cluster_sizes<<<g, 256, 0, c->stream>>>(c->p, sizes);
+        k_cluster_moments<<<g, 256, 0, c->stream>>>(c->p, sizes, out);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h, out, 16, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(sizes);
+    if (e != cudaSuccess) return cuda_fail(c, e, "sw_get_cluster_stats");
+    if (n_clusters) *n_clusters = h[0];
+    if (sum_nc2) *sum_nc2 = h[1];
+    return SW_OK;
+}
+
 int sw_get_counts(sw_ctx *c, int64_t *E, int64_t *M_or_nk, int n)
 {
     int rc = check_ctx(c);

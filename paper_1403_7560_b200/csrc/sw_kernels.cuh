@@ -1109,6 +1109,37 @@ __global__ void __launch_bounds__(256) k_measure_clock(const Params p)
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Cluster statistics of the last step's labelling, on request (sw_get_cluster_stats): the improved
+// estimator <M^2> = <sum_c n_c^2> of the FK representation ("easy to
+// extend").  k_cluster_sizes: every site adds 1 to the counter of its root; k_cluster_moments: number
+// of clusters and sum of squared sizes over the non-empty counters.  Not on the hot path.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_cluster_sizes(const Params p, uint32_t *sizes)
+{
+    const uint32_t a0 = blockIdx.x * 256u + threadIdx.x;  // tile-major address; N is a multiple of 1024
+    uint32_t a = a0;
+    const int db = p.db;
+    for (;;) {
+        const uint32_t n = p.labels[a] >> db;
+        if (n == a) break;
+        a = n;
+    }
+    atomicAdd(&sizes[a], 1u);
+}
+
+__global__ void __launch_bounds__(256) k_cluster_moments(const Params p, const uint32_t *sizes, unsigned long long *out)
+{
+    const uint32_t a = blockIdx.x * 256u + threadIdx.x;
+    const unsigned long long n = sizes[a];
+    unsigned long long cnt = n ? 1ull : 0ull, sq = n * n;
+    for (int o = 16; o > 0; o >>= 1) {
+        cnt += __shfl_down_sync(FULL, cnt, o);
+        sq += __shfl_down_sync(FULL, sq, o);
+    }
+    if ((threadIdx.x & 31) == 0 && cnt) { atomicAdd(&out[0], cnt); atomicAdd(&out[1], sq); }
+}
+
 // k_snapshot: copy the head of the accumulators (one record of a per-step series) -- sw_run_series:
 // w1 words from the start, then w2 words from word offset off2 (the clock model's D[d]).
 __global__ void __launch_bounds__(1024) k_snapshot(const Acc *acc, unsigned long long *dst, int w1, int off2, int w2)

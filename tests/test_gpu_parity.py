@@ -507,3 +507,34 @@ def test_clock_injected_states_series_and_full_size():
     Dg, ng = g.clock_hist()
     Do, no = o.clock_hist()
     assert np.array_equal(Dg, Do) and np.array_equal(ng, no)
+
+
+@pytest.mark.parametrize("dim,L,model,q,T", [(2, 64, 0, 0, TC2), (3, 32, 0, 0, T3), (2, 128, 1, 3, TP3), (3, 64, 0, 0, T3), (3, 32, 3, 16, 2.0)])
+def test_cluster_statistics_and_improved_estimator(dim, L, model, q, T):
+    """number of clusters and sum_c n_c^2 of the labelling, exact against the oracle
+    (and against numpy on the GPU's own labels); for Ising the FK identity <M^2> = <sum_c n_c^2> over a
+    run (3 sigma) ties the spins to the labels on the GPU itself."""
+    sw, orc = _mods()
+    from stats import binned_mean_err
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=8)
+    o = orc.Oracle(dim, L, model, q, 1.0 / T, 8)
+    for t in range(6):
+        g.step(1)
+        so_ = o.run_series(1)
+        ncl, s2 = g.cluster_stats()
+        lab = g.labels()
+        _, counts = np.unique(lab, return_counts=True)
+        assert ncl == len(counts) and s2 == int((counts.astype(np.int64) ** 2).sum())
+        assert ncl == int(so_["n_clusters"][0])
+        if model != 3:
+            assert s2 == int(so_["sum_nc2"][0])
+    if model == 0 and dim == 2:
+        m2, nc2 = [], []
+        g.step(300)
+        for _ in range(6000):
+            g.step(1)
+            nc2.append(g.cluster_stats()[1])       # clusters of this step's bonds (built on the previous spins)
+            m2.append(g.observables()[2])          # spins after this step
+        a, ea = binned_mean_err(np.array(m2, dtype=np.float64), 40)
+        b, eb = binned_mean_err(np.array(nc2, dtype=np.float64), 40)
+        assert abs(a - b) <= 3.0 * math.hypot(ea, eb), f"<M^2> = {a} +- {ea}, <sum n_c^2> = {b} +- {eb}"
