@@ -218,6 +218,16 @@ def oracle_baseline(cfg, spins, t, max_seconds=30.0):
                       f"{el:.1f} s on 1 thread of {os.cpu_count()} host cores", "ns_per_site": 1e9 * el / (n * done)}
 
 
+def max_over_ranks(ms, device):
+    """Replicas only: the job's step time is the slowest rank's; the one
+    collective of the multi-GPU path (not on the data path).  Works on NCCL (cuda) and gloo (cpu)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -244,9 +254,7 @@ def run_ours(args):
     with ClockSampler(local) as clk:
         g, ms, kms, flushed = time_config(sw, torch, cfg, args.seed + rank, burn, warm, args.steps, flush_buf)
     if world > 1:
-        tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms_all = float(tmax.item())
+        ms_all = max_over_ranks(ms, "cuda")
     else:
         ms_all = ms
     value = world * n_sites / (ms_all * 1e-3)

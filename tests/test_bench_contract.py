@@ -45,3 +45,34 @@ def test_ours_arm_fails_loudly_without_gpu():
     r = subprocess.run([sys.executable, "bench.py", "--steps", "1", "--warmup", "3", "--no-extras"],
                        cwd=ROOT, capture_output=True, text=True, timeout=600)
     assert r.returncode != 0 and "no CPU fallback" in (r.stderr + r.stdout)
+
+
+def _gloo_worker(rank, world, port, q):
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    r, w, l = bench.dist_env()
+    dist.barrier()
+    ms = bench.max_over_ranks(1.0 + rank, "cpu")      # rank 1 is the slower replica
+    dist.barrier()
+    dist.destroy_process_group()
+    q.put((rank, r, w, l, ms))
+
+
+def test_replica_timing_max_over_ranks_gloo_world2():
+    """The N > 1 path of bench.py is "replicas only": per-rank chains, a barrier, and the maximum of
+    the per-rank step times.  Exercised here with world_size 2 on the gloo backend (CPU)."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, 29747, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert [x[:4] for x in res] == [(0, 0, 2, 0), (1, 1, 2, 1)]
+    assert all(x[4] == 2.0 for x in res)
