@@ -1,6 +1,7 @@
 // sw_api.cu -- host driver and C ABI (include/sw.h) of libsw_b200.
 // Launch sequencing of one Swendsen-Wang step: k_bond_label -> k_merge -> k_flip,
-// all asynchronous on the context's stream; no host synchronisation inside sw_step.
+// all asynchronous on the context's stream (plain launches, or CUDA-graph replay for Ising / Potts on
+// any lattice size); no host synchronisation inside sw_step.
 #include "../../include/sw.h"
 #include "sw_kernels.cuh"
 

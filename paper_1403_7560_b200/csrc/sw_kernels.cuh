@@ -5,16 +5,19 @@
 //   k_bond_label  (1) bond activation fused with (2a) tile-local cluster labelling in
 //                 shared memory.  A thread owns "quads" of 4 consecutive sites along x (one 32-bit
 //                 spin word); x-connectivity is resolved with two warp ballots, y/z bonds inside the
-//                 tile by an atomicMin union-find in shared memory;
+//                 tile by a CAS hook round, pointer jumping and an atomicMin union-find for what
+//                 is left, all in shared memory; bonds through tile faces go to a global pair list;
 //   k_merge       (2b) global lock-free union-find (atomicCAS, min linear index wins) over the active
 //                 bonds that cross tile faces incl. the periodic wrap;
 //   k_flip        (2c) root chase fused with (3) the per-cluster new value / XY reflection
 //                  and the magnetisation sums of PAPER.md:142-157;
-//   k_measure     energy (Eq. 1-3) and magnetisation (Eq. 4, 5) of the current configuration.
+//   k_measure4 / k_measure / k_measure_clock   energy (Eq. 1-3) and magnetisation (Eq. 4, 5) of the
+//                 current configuration, on request (sw_observables, sw_run_series).
+// Models: Ising, q-state Potts, continuous XY, q-state clock (the discretisation the paper runs).
 //
 // Label array (HBM), one 32-bit word per site, TILE-MAJOR: the word of the site with tile-local
 // index li = lx + TX (ly + TY lz) in tile T lives at address a = T * NS + li, and holds
-//     (parent address << DB) | (the site's own cluster draw, DB bits: word 3 of its Philox call).
+//     (parent address << DB) | (the site's own cluster draw, DB bits, from its Philox call).
 // A site is a root iff parent address == own address.  Hooking always puts the root with the larger
 // LINEAR site index under the one with the smaller, so the final root of a cluster is its minimum
 // linear site index (what label equivalence with atomicMin from label = index converges to,
@@ -210,11 +213,14 @@ __global__ void __launch_bounds__(256) k_tile_origin(const Params p)
 // ------------------------------------------------------------------------------------------------
 // k_bond_label: one CTA per tile, QPT quads per thread.
 //   phase 0 (XY)  projections a_i = r . s_i of the tile and its three plus-faces into smem
-//   phase 1       per quad: spins of the quad and of its +x/+y/+z neighbours, one Philox call per
-//                 site, bond nibbles; two ballots give every site the start of its
-//                 x-run; label_s[site] = run start; face bonds -> face bit words
-//   phase 2       every thread walks the set bits of its y/z work mask: atomicMin union in smem
-//   phase 3       label word = (address of the tile-local root << DB) | own draw, 16-byte stores
+//   phase 1       per quad: spins of the quad and of its +x/+y/+z neighbours, the Philox call(s)
+//                 (reading 6), bond nibbles; two ballots give every site the
+//                 start of its x-run; label_s[site] = run start; face bonds -> face bit words
+//   phase 2a      hook round over the thread's active y/z bonds: CAS(larger root -> smaller root),
+//                 failures stay pending; two pointer-jumping steps
+//   phase 2b      pending bonds compacted into one list, handled by the general atomicMin union-find
+//   phase 3       two more jumping steps, label word = (address of the parent << DB) | own draw with
+//                 16-byte stores; active face bonds appended to the global pair list
 // ------------------------------------------------------------------------------------------------
 template <int DIM, int MODEL, int TX, int TY, int TZ, int NT>
 __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(const Params p)
