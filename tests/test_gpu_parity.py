@@ -538,3 +538,20 @@ def test_cluster_statistics_and_improved_estimator(dim, L, model, q, T):
         a, ea = binned_mean_err(np.array(m2, dtype=np.float64), 40)
         b, eb = binned_mean_err(np.array(nc2, dtype=np.float64), 40)
         assert abs(a - b) <= 3.0 * math.hypot(ea, eb), f"<M^2> = {a} +- {ea}, <sum n_c^2> = {b} +- {eb}"
+
+
+@pytest.mark.parametrize("dim,L,model,q,T", [(2, 128, 0, 0, TC2), (3, 64, 1, 3, 1.8), (3, 32, 2, 0, 2.2019), (2, 64, 3, 16, 0.9)])
+def test_checkpoint_resume(dim, L, model, q, T):
+    """the generator is counter-based, so (spins, seed, t) is the whole state: a chain
+    restored into a fresh context continues bit for bit."""
+    sw, _ = _mods()
+    a = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=12)
+    a.step(10)
+    spins, t = a.spins(), a.t
+    a.step(10)
+    b = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=12)
+    b.set_spins(spins, t)
+    b.step(10)
+    assert b.t == a.t == 20
+    assert np.array_equal(a.spins(), b.spins())
+    assert a.observables() == pytest.approx(b.observables(), rel=1e-12)
