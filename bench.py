@@ -367,7 +367,7 @@ def run_reference(args):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": warm, "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32" if cfg["model"] == 2 else ("u8" if cfg["model"] == 1 else "int8"),
+        "vs_baseline": None, "dtype": {0: "int8", 1: "u8", 2: "f32", 3: "u16"}[cfg["model"]],
         "data": "synthetic", "config": {"workload": f"{args.config}: {cfg['desc']} (oracle sample L={L})", "sites": n},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
