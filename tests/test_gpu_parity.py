@@ -555,3 +555,21 @@ def test_checkpoint_resume(dim, L, model, q, T):
     assert b.t == a.t == 20
     assert np.array_equal(a.spins(), b.spins())
     assert a.observables() == pytest.approx(b.observables(), rel=1e-12)
+
+
+def test_contexts_are_independent():
+    """Two contexts stepped in an interleaved fashion (same stream, and one with a library-owned
+    stream) give what each gives alone: the library keeps no state outside a context."""
+    sw, _ = _mods()
+    ref_a = sw.SwendsenWang(3, 64, 0, 0, 1.0 / T3, seed=21)
+    ref_b = sw.SwendsenWang(2, 256, 1, 3, 1.0 / TP3, seed=22)
+    ref_a.step(12)
+    ref_b.step(12)
+    a = sw.SwendsenWang(3, 64, 0, 0, 1.0 / T3, seed=21)
+    b = sw.SwendsenWang(2, 256, 1, 3, 1.0 / TP3, seed=22, use_torch=False)
+    for _ in range(6):
+        a.step(1)
+        b.step(2)
+        a.step(1)
+    assert np.array_equal(a.spins(), ref_a.spins()) and np.array_equal(b.spins(), ref_b.spins())
+    assert a.counts() == ref_a.counts() and b.counts() == ref_b.counts()
