@@ -93,7 +93,8 @@ int sw_observables(sw_ctx *c, double *host_E, double *host_M, double *host_M2, d
  * loop): the per-step sums stay on the device and are
  * copied out once at the end, so there is no host round trip per step.  host_E .. host_M4 are HOST
  * arrays of n doubles each (any may be NULL) with the same meaning as in sw_observables.  Needs
- * n x (5 + q) x 8 bytes of scratch device memory for the call (SW_ENOMEM if that fails). */
+ * n x (5 + q) x 8 bytes (clock: 5 + 2q) of library-owned device memory, allocated on first use, kept
+ * with the context and grown when a larger n is asked for (SW_ENOMEM if that fails). */
 int sw_run_series(sw_ctx *c, int n, double *host_E, double *host_M, double *host_M2, double *host_M4);
 
 /* Destroy the context (synchronises its stream first).  NULL is a no-op. */

@@ -181,6 +181,8 @@ struct sw_ctx {
     // CUDA graphs of 1 and GRAPH_STEPS consecutive steps (3 kernel nodes per step); built lazily for
     // Ising / Potts, rebuilt when the bond-recording flag changes.  XY passes a new direction with
     // every step and keeps plain launches.
+    unsigned long long *series_dev;   // sw_run_series: device records, kept and grown on demand
+    size_t series_cap;                // in 64-bit words
     cudaGraphExec_t graph1, graphK;
     int graph_record;   // record_bonds state the graphs were built for (-1: none)
     bool own_workspace, own_stream;
@@ -419,6 +421,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     p.counting = 0;
     c->force_phi = 0; c->forced_phi = 0.0; c->rx = c->ry = c->crefl = 0.f; c->sticky = 0;
     c->graph1 = nullptr; c->graphK = nullptr; c->graph_record = -1;
+    c->series_dev = nullptr; c->series_cap = 0;
     c->timing = 0; c->timed_steps = 0;
     for (int k = 0; k < 3; ++k) c->kernel_ms[k] = 0.0;
     for (int k = 0; k < 4; ++k) c->ev[k] = nullptr;
@@ -627,9 +630,18 @@ int sw_run_series(sw_ctx *c, int n, double *E, double *M, double *M2, double *M4
     // per step one record of 5 + q 64-bit words = the head of Acc (E_int, E_xy, M_int, mx, my, n_k)
     const int w1 = 5 + c->q, w2 = (c->model == SW_CLOCK) ? c->q : 0, words = w1 + w2;
     const int off2 = (int)(offsetof(Acc, dk) / 8);
-    unsigned long long *dser = nullptr;
-    cudaError_t e = cudaMalloc(&dser, (size_t)n * words * 8);
-    if (e != cudaSuccess) { cudaGetLastError(); return fail(SW_ENOMEM, "sw_run_series: cudaMalloc of the series buffer failed"); }
+    cudaError_t e = cudaSuccess;
+    if (c->series_cap < (size_t)n * words) {
+        // (re)allocate the record buffer; it stays with the context, so that calling this in a loop
+        // costs no cudaMalloc / cudaFree (both synchronise the device)
+        SW_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (c->series_dev) cudaFree(c->series_dev);
+        c->series_dev = nullptr; c->series_cap = 0;
+        e = cudaMalloc(&c->series_dev, (size_t)n * words * 8);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(SW_ENOMEM, "sw_run_series: cudaMalloc of the series buffer failed"); }
+        c->series_cap = (size_t)n * words;
+    }
+    unsigned long long *dser = c->series_dev;
     for (int s = 0; s < n && rc == SW_OK; ++s) {
         rc = sw_step(c, 1);
         if (rc == SW_OK) rc = refresh_observables(c);
@@ -662,7 +674,6 @@ int sw_run_series(sw_ctx *c, int n, double *E, double *M, double *M2, double *M4
         }
     }
     std::free(hser);
-    cudaFree(dser);
     return rc;
 }
 
@@ -670,6 +681,7 @@ int sw_destroy(sw_ctx *c)
 {
     if (!c) return SW_OK;
     cudaStreamSynchronize(c->stream);
+    if (c->series_dev) cudaFree(c->series_dev);
     if (c->graph1) cudaGraphExecDestroy(c->graph1);
     if (c->graphK) cudaGraphExecDestroy(c->graphK);
     for (int k = 0; k < 4; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
