@@ -304,7 +304,7 @@ def run_ours(args):
         # the paper's second row (Table 1): update + measurement of E and M every step,
         # through sw_run_series (per-step sums stay on the device)
         ns = max(3, min(args.steps, 20))
-        g.run_series(3)
+        g.run_series(ns)   # warm-up with the same length: the record buffer is sized once
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
