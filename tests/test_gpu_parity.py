@@ -573,3 +573,22 @@ def test_contexts_are_independent():
         a.step(1)
     assert np.array_equal(a.spins(), ref_a.spins()) and np.array_equal(b.spins(), ref_b.spins())
     assert a.counts() == ref_a.counts() and b.counts() == ref_b.counts()
+
+
+@pytest.mark.parametrize("dim,L,model,q,T", [(3, 128, 0, 0, T3), (2, 1024, 0, 0, TC2), (3, 96, 3, 64, 2.2)])
+def test_repeated_step_is_deterministic(dim, L, model, q, T):
+    """The lock-free union-finds run in a different order every time; the result must not depend on it:
+    the same step from the same state, 12 times, gives identical labels and spins (I6)."""
+    sw, _ = _mods()
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=31)
+    g.step(40)
+    state, t = g.spins(), g.t
+    ref_labels = ref_spins = None
+    for k in range(12):
+        g.set_spins(state, t)
+        g.step(1)
+        labels, spins = g.labels(), g.spins()
+        if k == 0:
+            ref_labels, ref_spins = labels, spins
+        else:
+            assert np.array_equal(labels, ref_labels) and np.array_equal(spins, ref_spins), f"repeat {k} differs"
