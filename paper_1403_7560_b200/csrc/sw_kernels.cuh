@@ -393,64 +393,57 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                 constexpr uint32_t FM = (1u << F) - 1u;
                 constexpr int SH2 = (DIM == 3) ? 2 * F - 32 : 0;  // field 2 inside the high word
                 const uint32_t Ptop = p.P32 >> (32 - F);
-                // d = field - Ptop (both < 2^21): the sign bit of d is "field < Ptop", and d == 0 is a tie.
-                // Sites are taken 3..0, one generator call at a time (low register pressure); the sign
-                // bits are shifted into the nibbles with one funnel shift each, and the minimum of all d
-                // tells whether any field of the quad sits on the threshold.
-                rnx = rny = 0u;
-                d = 0u;
-                uint32_t dmin = 0xffffffffu;
+                uint32_t f0[4], f1[4], f2[4];
                 if (DIM == 2) {
                     const uint4 c = philox4x32_10(g >> 2, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
                     const uint32_t cw[4] = {c.x, c.y, c.z, c.w};
+                    d = 0u;
 #pragma unroll
-                    for (int s = 3; s >= 0; --s) {
-                        const uint32_t d0 = (cw[s] & FM) - Ptop, d1 = ((cw[s] >> F) & FM) - Ptop;
-                        rnx = __funnelshift_l(d0, rnx, 1);
-                        rny = __funnelshift_l(d1, rny, 1);
-                        d = __funnelshift_l(cw[s], d, 1);
-                        dmin = min(dmin, min(d0, d1));
+                    for (int s = 0; s < 4; ++s) {
+                        f0[s] = cw[s] & FM; f1[s] = (cw[s] >> F) & FM; f2[s] = 0u;
+                        d |= (cw[s] >> 31) << s;
                     }
                 } else {
+                    const uint4 c0 = philox4x32_10(g >> 1, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
+                    const uint4 c1 = philox4x32_10((g >> 1) + 1u, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
+                    const uint32_t lo[4] = {c0.x, c0.z, c1.x, c1.z}, hi[4] = {c0.y, c0.w, c1.y, c1.w};
+                    d = 0u;
 #pragma unroll
-                    for (int h = 1; h >= 0; --h) {
-                        const uint4 c = philox4x32_10((g >> 1) + h, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
-                        const uint32_t lo[2] = {c.x, c.z}, hi[2] = {c.y, c.w};
+                    for (int s = 0; s < 4; ++s) {
+                        f0[s] = lo[s] & FM;
+                        f1[s] = __funnelshift_r(lo[s], hi[s], F) & FM;
+                        f2[s] = (hi[s] >> SH2) & FM;
+                        d |= (hi[s] >> 31) << s;
+                    }
+                }
+                // d = field - Ptop (both < 2^21): the sign bit of d is "field < Ptop", and d == 0 is a tie.
+                // Sign bits are shifted into the nibbles with one funnel shift each (sites 3..0), and the
+                // minimum of all d tells whether any field of the quad sits on the threshold.
+                rnx = rny = 0u;
+                uint32_t dmin = 0xffffffffu;
 #pragma unroll
-                        for (int u = 1; u >= 0; --u) {
-                            const uint32_t d0 = (lo[u] & FM) - Ptop;
-                            const uint32_t d1 = (__funnelshift_r(lo[u], hi[u], F) & FM) - Ptop;
-                            const uint32_t d2 = ((hi[u] >> SH2) & FM) - Ptop;
-                            rnx = __funnelshift_l(d0, rnx, 1);
-                            rny = __funnelshift_l(d1, rny, 1);
-                            rnz = __funnelshift_l(d2, rnz, 1);
-                            d = __funnelshift_l(hi[u], d, 1);
-                            dmin = min(dmin, min(d0, min(d1, d2)));
-                        }
+                for (int s = 3; s >= 0; --s) {
+                    const uint32_t d0 = f0[s] - Ptop, d1 = f1[s] - Ptop;
+                    rnx = __funnelshift_l(d0, rnx, 1);
+                    rny = __funnelshift_l(d1, rny, 1);
+                    dmin = min(dmin, min(d0, d1));
+                    if (DIM == 3) {
+                        const uint32_t d2 = f2[s] - Ptop;
+                        rnz = __funnelshift_l(d2, rnz, 1);
+                        dmin = min(dmin, d2);
                     }
                 }
                 if (dmin == 0u) {  // probability 12 x 2^-21 per quad (3D), 8 x 2^-15 (2D)
-                    // rare: redo the quad site by site from the generator (nothing is kept in registers
-                    // for this path) and settle the tied bonds with the TIE call of their site
+                    // fully unrolled: the field arrays are only ever indexed statically (registers)
                     const uint32_t Plow = p.P32 & ((1u << (32 - F)) - 1u);
-#pragma unroll 1
+#pragma unroll
                     for (int s = 0; s < 4; ++s) {
-                        const uint32_t i = g + s;
-                        uint32_t e0, e1, e2 = ~0u;
-                        if (DIM == 2) {
-                            const uint4 c = philox4x32_10(i >> 2, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
-                            const uint32_t w1 = (s == 0) ? c.x : (s == 1) ? c.y : (s == 2) ? c.z : c.w;
-                            e0 = w1 & FM; e1 = (w1 >> F) & FM;
-                        } else {
-                            const uint4 c = philox4x32_10(i >> 1, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
-                            const uint32_t l1 = (s & 1) ? c.z : c.x, h1 = (s & 1) ? c.w : c.y;
-                            e0 = l1 & FM; e1 = __funnelshift_r(l1, h1, F) & FM; e2 = (h1 >> SH2) & FM;
-                        }
-                        if (e0 == Ptop || e1 == Ptop || e2 == Ptop) {
-                            const uint4 tw = philox4x32_10(i, t_lo, t_hi, DOM_TIE, p.k0, p.k1);
-                            if (e0 == Ptop && (tw.x >> F) < Plow) rnx |= 1u << s;
-                            if (e1 == Ptop && (tw.y >> F) < Plow) rny |= 1u << s;
-                            if (DIM == 3 && e2 == Ptop && (tw.z >> F) < Plow) rnz |= 1u << s;
+                        const bool t0 = f0[s] == Ptop, t1 = f1[s] == Ptop, t2 = DIM == 3 && f2[s] == Ptop;
+                        if (t0 || t1 || t2) {
+                            const uint4 tw = philox4x32_10(g + s, t_lo, t_hi, DOM_TIE, p.k0, p.k1);
+                            if (t0 && (tw.x >> F) < Plow) rnx |= 1u << s;
+                            if (t1 && (tw.y >> F) < Plow) rny |= 1u << s;
+                            if (t2 && (tw.z >> F) < Plow) rnz |= 1u << s;
                         }
                     }
                 }
