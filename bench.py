@@ -65,7 +65,7 @@ def kernel_bytes_per_site(model):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the one
 # `ncu --set full` capture summarised in profiles/r01_final_ncu_full_C4.md (config -> kernel -> bytes).
-NCU_TRAFFIC = {"C4": {"k_bond_label": 134.6e6 + 520.7e6, "k_merge": 635.8e6 + 120.8e6, "k_flip": 538.0e6 + 120.9e6}}
+NCU_TRAFFIC = {"C4": {"k_bond_label": 134.6e6 + 523.6e6, "k_merge": 636.0e6 + 121.3e6, "k_flip": 538.0e6 + 120.5e6}}
 
 
 class ClockSampler:
