@@ -67,6 +67,7 @@ bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
     SW_TILE3(32, 16, 8)
     SW_TILE3(32, 16, 16)
     SW_TILE3(64, 8, 8)
+    if (dim == 3 && tx == 32 && ty == 32 && tz == 16) { o = make_ops<3, MODEL, 32, 32, 16, 8>(); return true; }  // 8 quads per thread
 #undef SW_TILE2
 #undef SW_TILE3
     return false;
@@ -113,6 +114,9 @@ void default_tile(int dim, int L, int model, int &tx, int &ty, int &tz)
         else { tx = 32; ty = 32; }
     } else {
         tx = 32; ty = 16; tz = 16;  // also for XY (75 KB of shared memory per CTA: projections + labels)
+        // Ising on very large lattices: 32x32x16 tiles with 8 quads per thread -- a fifth fewer bonds
+        // through tile faces, measured 2 % ahead at L = 512 (behind at L = 256 and for the other models)
+        if (model == SW_ISING && (double)L * L * L >= 134217728.0) ty = 32;
     }
 }
 

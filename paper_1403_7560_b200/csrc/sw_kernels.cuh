@@ -171,6 +171,14 @@ __device__ __forceinline__ void union_s(uint32_t *lab, uint32_t a, uint32_t b)
     }
 }
 
+// The per-thread mask of pending y/z bonds: 32 bits, or 64 when a thread owns 8 quads in 3D.
+template <bool WIDE> struct WorkWord { using type = uint32_t; };
+template <> struct WorkWord<true> { using type = unsigned long long; };
+__device__ __forceinline__ int ffs_w(uint32_t v) { return __ffs(v); }
+__device__ __forceinline__ int ffs_w(unsigned long long v) { return __ffsll((long long)v); }
+__device__ __forceinline__ uint32_t popc_w(uint32_t v) { return __popc(v); }
+__device__ __forceinline__ uint32_t popc_w(unsigned long long v) { return __popcll(v); }
+
 // One pointer-jumping step for the 4 sites of a quad: r <- parent(r) where the previous step still
 // moved (r != prev); a site that has reached a fixed point (a root) issues no load, so roots and
 // their direct children cost no shared-memory wavefronts.
@@ -229,7 +237,8 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     constexpr int NS = G::NS, NQ = NS / 4, QPT = NQ / NT, LPR = TX / 4;
     constexpr int WB = (DIM == 3) ? 8 : 4;  // work bits per quad: 4 y bonds (+ 4 z bonds)
     static_assert(NQ % NT == 0 && NT % 32 == 0, "whole quads per thread, whole rows per warp");
-    static_assert(QPT * WB <= 32, "the work mask of a thread is one 32-bit word");
+    static_assert(QPT * WB <= 64, "the work mask of a thread is one 32- or 64-bit word");
+    using work_t = typename WorkWord<(QPT * WB > 32)>::type;
     extern __shared__ __align__(16) uint32_t smem_u32[];
     static_assert(G::NFW <= 64, "two face words per lane of warp 0");
     static_assert(NS <= 32768, "a leftover entry keeps the site in 15 bits");
@@ -292,7 +301,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
 
     uint32_t bnd[QPT];   // per quad: bits 0-3 x bonds, 4-7 y bonds, 8-11 z bonds
     uint32_t drw[QPT];   // per quad: the four draws, DB bits each (site s at bit s * db)
-    uint32_t work = 0u;  // per quad WB bits: y (and z) bonds that stay inside the tile
+    work_t work = 0;  // per quad WB bits: y (and z) bonds that stay inside the tile
     const int db = (MODEL == POTTS) ? p.db : 1;
 
 #pragma unroll
@@ -497,7 +506,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
         }
         uint32_t wk = (ly < TY - 1) ? byn : 0u;
         if (DIM == 3 && lz < TZ - 1) wk |= bzn << 4;
-        work |= wk << (j * WB);
+        work |= (work_t)wk << (j * WB);
     }
     __syncthreads();
 
@@ -529,17 +538,17 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
         if (SW_BL_HOOK_LOOP && DIM == 3) {
             // one iteration per active bond of the thread (trip count = the largest popcount in the
             // warp): at 3D densities (a quarter of the bond slots active) this beats the predicated code
-            uint32_t todo = work;
-            work = 0u;
-            while (__any_sync(FULL, todo != 0u)) {
+            work_t todo = work;
+            work = 0;
+            while (__any_sync(FULL, todo != 0)) {
                 if (todo) {
-                    const int k = __ffs(todo) - 1;
-                    todo &= todo - 1u;
+                    const int k = ffs_w(todo) - 1;
+                    todo &= todo - 1;
                     const uint32_t a = (uint32_t)((tid + (k / WB) * NT) * 4 + (k & 3));
                     const uint32_t b = a + (((k % WB) & 4) ? (uint32_t)(TX * TY) : (uint32_t)TX);
                     const uint32_t pa = lab_s[a], pb = lab_s[b];
                     const uint32_t hi = max(pa, pb), lo = min(pa, pb);
-                    if (hi != lo && atomicCAS(&lab_s[hi], hi, lo) != hi) work |= 1u << k;
+                    if (hi != lo && atomicCAS(&lab_s[hi], hi, lo) != hi) work |= (work_t)1 << k;
                 }
             }
         } else {
@@ -550,7 +559,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
             const uint32_t av[4] = {la.x, la.y, la.z, la.w};
 #pragma unroll
             for (int dir = 0; dir < (DIM == 3 ? 2 : 1); ++dir) {
-                const uint32_t nib = (work >> (j * WB + 4 * dir)) & 0xfu;
+                const uint32_t nib = (uint32_t)(work >> (j * WB + 4 * dir)) & 0xfu;
                 const uint4 lb = *reinterpret_cast<const uint4 *>(lab_s + ((li + (dir ? TX * TY : TX)) & (NS - 1)));
                 const uint32_t bv[4] = {lb.x, lb.y, lb.z, lb.w};
                 uint32_t left = 0u;
@@ -564,7 +573,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                                  : "+r"(old) : "r"(lab_sa + 4u * hi), "r"(hi), "r"(lo), "r"(need) : "memory");
                     left |= (uint32_t)(old != hi) << sidx;
                 }
-                work = (work & ~(0xfu << (j * WB + 4 * dir))) | (left << (j * WB + 4 * dir));
+                work = (work & ~((work_t)0xfu << (j * WB + 4 * dir))) | ((work_t)left << (j * WB + 4 * dir));
             }
         }
         }
@@ -585,7 +594,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     // through the general union-find.  The leftovers of all threads are first compacted into one list
     // so that every lane of every warp has a union to do (a warp whose entries do not fit keeps them).
     if (SW_BL_ROUNDS > 0) {
-        const uint32_t cnt = __popc(work);
+        const uint32_t cnt = popc_w(work);
         uint32_t inc = cnt;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -599,8 +608,8 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
         if (tot && base + tot <= (uint32_t)G::LEFT_CAP) {
             uint32_t pos = base + inc - cnt;
             while (work) {
-                const int k = __ffs(work) - 1;
-                work &= work - 1u;
+                const int k = ffs_w(work) - 1;
+                work &= work - 1;
                 const int jq = k / WB, r = k % WB;
                 left_s[pos++] = (uint16_t)(((tid + jq * NT) * 4 + (r & 3)) | ((r & 4) << 13));
             }
@@ -622,10 +631,10 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     }
     // warp-uniform trip count + __syncwarp: lanes whose union ends early wait for the others instead
     // of drifting into later iterations on their own (that would serialise the warp)
-    while (__any_sync(FULL, work != 0u)) {
+    while (__any_sync(FULL, work != 0)) {
         if (work) {
-            const int k = __ffs(work) - 1;
-            work &= work - 1u;
+            const int k = ffs_w(work) - 1;
+            work &= work - 1;
             const int jq = k / WB, r = k % WB;
             const uint32_t a = (uint32_t)((tid + jq * NT) * 4 + (r & 3));
             union_s(lab_s, a, a + ((r & 4) ? (uint32_t)(TX * TY) : (uint32_t)TX));

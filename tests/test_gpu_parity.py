@@ -95,7 +95,7 @@ def test_tile_menu_2d(tile, monkeypatch):
         _compare_step(g, o, f"tile {tile} t={t}")
 
 
-@pytest.mark.parametrize("tile", ["32x8x8", "32x16x8", "32x16x16", "64x8x8"])
+@pytest.mark.parametrize("tile", ["32x8x8", "32x16x8", "32x16x16", "64x8x8", "32x32x16"])
 def test_tile_menu_3d(tile, monkeypatch):
     sw, orc = _mods()
     monkeypatch.setenv("SW_B200_TILE", tile)
