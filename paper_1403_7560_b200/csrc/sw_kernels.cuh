@@ -548,7 +548,10 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                     const uint32_t b = a + (((k % WB) & 4) ? (uint32_t)(TX * TY) : (uint32_t)TX);
                     const uint32_t pa = lab_s[a], pb = lab_s[b];
                     const uint32_t hi = max(pa, pb), lo = min(pa, pb);
-                    if (hi != lo && atomicCAS(&lab_s[hi], hi, lo) != hi) work |= (work_t)1 << k;
+                    if (hi != lo) {
+                        const uint32_t old = atomicCAS(&lab_s[hi], hi, lo);
+                        if (old != hi && old != lo) work |= (work_t)1 << k;  // old == lo: a twin bond did it already
+                    }
                 }
             }
         } else {
@@ -571,7 +574,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
                                  "@p atom.shared.cas.b32 %0, [%1], %2, %3;\n\t}"
                                  : "+r"(old) : "r"(lab_sa + 4u * hi), "r"(hi), "r"(lo), "r"(need) : "memory");
-                    left |= (uint32_t)(old != hi) << sidx;
+                    left |= (uint32_t)(old != hi && old != lo) << sidx;  // old == lo: a twin bond did it already
                 }
                 work = (work & ~((work_t)0xfu << (j * WB + 4 * dir))) | ((work_t)left << (j * WB + 4 * dir));
             }
