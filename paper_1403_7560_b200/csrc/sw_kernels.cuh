@@ -171,13 +171,6 @@ __device__ __forceinline__ void union_s(uint32_t *lab, uint32_t a, uint32_t b)
     }
 }
 
-// The per-thread mask of pending y/z bonds: 32 bits, or 64 when a thread owns 8 quads in 3D.
-template <bool WIDE> struct WorkWord { using type = uint32_t; };
-template <> struct WorkWord<true> { using type = unsigned long long; };
-__device__ __forceinline__ int ffs_w(uint32_t v) { return __ffs(v); }
-__device__ __forceinline__ int ffs_w(unsigned long long v) { return __ffsll((long long)v); }
-__device__ __forceinline__ uint32_t popc_w(uint32_t v) { return __popc(v); }
-__device__ __forceinline__ uint32_t popc_w(unsigned long long v) { return __popcll(v); }
 
 // One pointer-jumping step for the 4 sites of a quad: r <- parent(r) where the previous step still
 // moved (r != prev); a site that has reached a fixed point (a root) issues no load, so roots and
@@ -235,10 +228,8 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
 {
     using G = TileGeom<DIM, TX, TY, TZ>;
     constexpr int NS = G::NS, NQ = NS / 4, QPT = NQ / NT, LPR = TX / 4;
-    constexpr int WB = (DIM == 3) ? 8 : 4;  // work bits per quad: 4 y bonds (+ 4 z bonds)
     static_assert(NQ % NT == 0 && NT % 32 == 0, "whole quads per thread, whole rows per warp");
-    static_assert(QPT * WB <= 64, "the work mask of a thread is one 32- or 64-bit word");
-    using work_t = typename WorkWord<(QPT * WB > 32)>::type;
+    static_assert(QPT * 4 <= 32, "the pending y bonds (and the pending z bonds) of a thread are one 32-bit mask");
     extern __shared__ __align__(16) uint32_t smem_u32[];
     static_assert(G::NFW <= 64, "two face words per lane of warp 0");
     static_assert(NS <= 32768, "a leftover entry keeps the site in 15 bits");
@@ -301,7 +292,9 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
 
     uint32_t bnd[QPT];   // per quad: bits 0-3 x bonds, 4-7 y bonds, 8-11 z bonds
     uint32_t drw[QPT];   // per quad: the four draws, DB bits each (site s at bit s * db)
-    work_t work = 0;  // per quad WB bits: y (and z) bonds that stay inside the tile
+    // pending bonds that stay inside the tile: bit 4 j + s = site s of the thread's quad j, one mask for
+    // the y bonds and one for the z bonds (32-bit masks, and the neighbour offset is a constant per mask)
+    uint32_t work[2] = {0u, 0u};
     const int db = (MODEL == POTTS) ? p.db : 1;
 
 #pragma unroll
@@ -504,9 +497,8 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
             const int b = lx + TX * ly;
             atomicOr(&face_s[G::FXW + G::FYW + (b >> 5)], bzn << (b & 31));
         }
-        uint32_t wk = (ly < TY - 1) ? byn : 0u;
-        if (DIM == 3 && lz < TZ - 1) wk |= bzn << 4;
-        work |= (work_t)wk << (j * WB);
+        if (ly < TY - 1) work[0] |= byn << (4 * j);
+        if (DIM == 3 && lz < TZ - 1) work[1] |= bzn << (4 * j);
     }
     __syncthreads();
 
@@ -538,19 +530,21 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
         if (SW_BL_HOOK_LOOP && DIM == 3) {
             // one iteration per active bond of the thread (trip count = the largest popcount in the
             // warp): at 3D densities (a quarter of the bond slots active) this beats the predicated code
-            work_t todo = work;
-            work = 0;
-            while (__any_sync(FULL, todo != 0)) {
-                if (todo) {
-                    const int k = ffs_w(todo) - 1;
-                    todo &= todo - 1;
-                    const uint32_t a = (uint32_t)((tid + (k / WB) * NT) * 4 + (k & 3));
-                    const uint32_t b = a + (((k % WB) & 4) ? (uint32_t)(TX * TY) : (uint32_t)TX);
-                    const uint32_t pa = lab_s[a], pb = lab_s[b];
-                    const uint32_t hi = max(pa, pb), lo = min(pa, pb);
-                    if (hi != lo) {
-                        const uint32_t old = atomicCAS(&lab_s[hi], hi, lo);
-                        if (old != hi && old != lo) work |= (work_t)1 << k;  // old == lo: a twin bond did it already
+#pragma unroll
+            for (int dir = 0; dir < 2; ++dir) {
+                uint32_t todo = work[dir];
+                work[dir] = 0u;
+                while (__any_sync(FULL, todo != 0u)) {
+                    if (todo) {
+                        const uint32_t k = 31u - (uint32_t)__clz((int)(todo & (0u - todo)));
+                        todo &= todo - 1u;
+                        const uint32_t a = (uint32_t)tid * 4u + (k >> 2) * (uint32_t)(NT * 4) + (k & 3u);
+                        const uint32_t pa = lab_s[a], pb = lab_s[a + (dir ? TX * TY : TX)];
+                        const uint32_t hi = max(pa, pb), lo = min(pa, pb);
+                        if (hi != lo) {
+                            const uint32_t old = atomicCAS(&lab_s[hi], hi, lo);
+                            if (old != hi && old != lo) work[dir] |= 1u << k;  // old == lo: a twin bond did it already
+                        }
                     }
                 }
             }
@@ -562,7 +556,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
             const uint32_t av[4] = {la.x, la.y, la.z, la.w};
 #pragma unroll
             for (int dir = 0; dir < (DIM == 3 ? 2 : 1); ++dir) {
-                const uint32_t nib = (uint32_t)(work >> (j * WB + 4 * dir)) & 0xfu;
+                const uint32_t nib = (work[dir] >> (4 * j)) & 0xfu;
                 const uint4 lb = *reinterpret_cast<const uint4 *>(lab_s + ((li + (dir ? TX * TY : TX)) & (NS - 1)));
                 const uint32_t bv[4] = {lb.x, lb.y, lb.z, lb.w};
                 uint32_t left = 0u;
@@ -576,7 +570,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                                  : "+r"(old) : "r"(lab_sa + 4u * hi), "r"(hi), "r"(lo), "r"(need) : "memory");
                     left |= (uint32_t)(old != hi && old != lo) << sidx;  // old == lo: a twin bond did it already
                 }
-                work = (work & ~((work_t)0xfu << (j * WB + 4 * dir))) | ((work_t)left << (j * WB + 4 * dir));
+                work[dir] = (work[dir] & ~(0xfu << (4 * j))) | (left << (4 * j));
             }
         }
         }
@@ -597,7 +591,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     // through the general union-find.  The leftovers of all threads are first compacted into one list
     // so that every lane of every warp has a union to do (a warp whose entries do not fit keeps them).
     if (SW_BL_ROUNDS > 0) {
-        const uint32_t cnt = popc_w(work);
+        const uint32_t cnt = __popc(work[0]) + __popc(work[1]);
         uint32_t inc = cnt;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -610,11 +604,15 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
         base = __shfl_sync(FULL, base, 31);
         if (tot && base + tot <= (uint32_t)G::LEFT_CAP) {
             uint32_t pos = base + inc - cnt;
-            while (work) {
-                const int k = ffs_w(work) - 1;
-                work &= work - 1;
-                const int jq = k / WB, r = k % WB;
-                left_s[pos++] = (uint16_t)(((tid + jq * NT) * 4 + (r & 3)) | ((r & 4) << 13));
+#pragma unroll
+            for (int dir = 0; dir < (DIM == 3 ? 2 : 1); ++dir) {
+                uint32_t w = work[dir];
+                while (w) {
+                    const uint32_t k = 31u - (uint32_t)__clz((int)(w & (0u - w)));
+                    w &= w - 1u;
+                    left_s[pos++] = (uint16_t)(((uint32_t)tid * 4u + (k >> 2) * (uint32_t)(NT * 4) + (k & 3u)) | (dir ? 0x8000u : 0u));
+                }
+                work[dir] = 0u;
             }
         } else if (tot && lane == 31) {
             atomicMin(&fpre_s[G::NFWP + 2], base);  // the list is valid below the first range that did not fit
@@ -634,15 +632,18 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     }
     // warp-uniform trip count + __syncwarp: lanes whose union ends early wait for the others instead
     // of drifting into later iterations on their own (that would serialise the warp)
-    while (__any_sync(FULL, work != 0)) {
-        if (work) {
-            const int k = ffs_w(work) - 1;
-            work &= work - 1;
-            const int jq = k / WB, r = k % WB;
-            const uint32_t a = (uint32_t)((tid + jq * NT) * 4 + (r & 3));
-            union_s(lab_s, a, a + ((r & 4) ? (uint32_t)(TX * TY) : (uint32_t)TX));
+#pragma unroll
+    for (int dir = 0; dir < (DIM == 3 ? 2 : 1); ++dir) {
+        uint32_t w = work[dir];
+        while (__any_sync(FULL, w != 0u)) {
+            if (w) {
+                const uint32_t k = 31u - (uint32_t)__clz((int)(w & (0u - w)));
+                w &= w - 1u;
+                const uint32_t a = (uint32_t)tid * 4u + (k >> 2) * (uint32_t)(NT * 4) + (k & 3u);
+                union_s(lab_s, a, a + (dir ? (uint32_t)(TX * TY) : (uint32_t)TX));
+            }
+            __syncwarp();
         }
-        __syncwarp();
     }
     __syncthreads();
 
