@@ -403,13 +403,17 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     p.ntz = (dim == 3) ? (uint32_t)(L / c->ops.tz) : 1u;
     p.ntiles = p.ntx * p.nty * p.ntz;
     p.db = draw_bits(model, q);
-    {   // k_merge: a resident grid that strides over the pair list
+    {   // k_merge: grid-stride loop over the pair list.  The grid is fixed at create time (graph replay) from
+        // the capacity of the list; 64 CTAs per SM leave one or two pairs per thread at T_c, so that CTAs
+        // run through the list in order (the list is in tile order: neighbouring pairs touch neighbouring
+        // label blocks, which stay in L2).  A resident grid (8 CTAs per SM, 13 pairs per thread) sweeps the
+        // whole label array 13 times instead: C4 k_merge 0.264 ms vs 0.138 ms.
         int dev = 0, sms = 148;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         const size_t max_pairs = c->N / c->ops.tx + c->N / c->ops.ty + (dim == 3 ? c->N / c->ops.tz : 0);
         size_t blocks = (max_pairs + 255) / 256;
-        if (blocks > (size_t)sms * 8) blocks = (size_t)sms * 8;
+        if (blocks > (size_t)sms * 64) blocks = (size_t)sms * 64;
         c->merge_blocks = (unsigned)blocks;
     }
     p.L = (uint32_t)L; p.N = (uint32_t)c->N;
