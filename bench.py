@@ -65,7 +65,7 @@ def kernel_bytes_per_site(model):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the one
 # `ncu --set full` capture summarised in profiles/r01_final_ncu_full_C4.md (config -> kernel -> bytes).
-NCU_TRAFFIC = {"C4": {"k_bond_label": 134.7e6 + 630.1e6, "k_merge": 505.2e6 + 89.2e6, "k_flip": 537.9e6 + 119.8e6}}
+NCU_TRAFFIC = {"C4": {"k_bond_label": 134.7e6 + 630.1e6, "k_merge": 380.1e6 + 74.6e6, "k_flip": 537.9e6 + 119.8e6}}
 
 
 class ClockSampler:
