@@ -40,15 +40,26 @@ void swo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* Reading 6: key = (seed low, seed high); counter = (index, t low, t high, domain).
- * Domain SITE (Potts, XY): one call per site and step, index = site; word k (k < dim) decides the
- * bond in direction k, word 3 is the new value of the cluster whose root (minimum site index) is
- * this site.
- * Domain PACK (Ising): the 128 bits of one call serve S consecutive sites, index = site / S, with
- * S = 4 in 2D and S = 2 in 3D; see ising_site_bits().  Domain TIE (Ising): index = site, word k
- * settles bond k when its PACK field sits exactly on the threshold.
- * Domain INIT: start configuration, word 0.  Domain XYDIR: the XY direction of step t, word 0. */
-enum { DOM_SITE = 0, DOM_PACK = 1, DOM_INIT = 2, DOM_XYDIR = 3, DOM_TIE = 4 };
+/* Reading 6 (revised in round 2): key = (seed low, seed high); counter = (index, t low,
+ * t high, domain).
+ * Domain SITE (XY, clock): one call per site and step, index = site; word k (k < dim) decides the
+ * bond in direction k, word 3 is the draw of the cluster whose root (minimum site index) is this site.
+ * Domain GROUP (Ising, Potts -- the two models whose bond probability is one constant): the 32
+ * sites with linear index 32 G .. 32 G + 31 (group G = site / 32, position b = site % 32) share one
+ * stream of words W_G[n], n = 0, 1, 2, ...:
+ *     W_G[n] = word n % 4 of the call with counter (G, t low, t high, GROUP + 256 (n / 4)).
+ *   W_G[0]               bit b: Ising, the new value of the cluster whose root is site b of the group
+ *   W_G[1 + s dim + k]   bit b: bit 31 - s (s = 0 is the most significant) of the 32-bit uniform
+ *                        integer u(site, k) that decides bond k of the site, s = 0 .. 31
+ *   W_G[128 + b]         Potts: the draw word of site b of the group
+ * i.e. the uniform integers of a group are stored transposed, one word per binary digit, so that a
+ * comparison u < P32 can be carried out for 32 sites at once, most significant digit first, and
+ * stopped as soon as every site is decided.  The decision itself is the plain one of reading 16:
+ * a bond between aligned neighbours is active iff u < P32.
+ * Domain INIT: start configuration, word 0.  Domain XYDIR: the XY direction of step t, word 0.
+ * (Domains 1 and 4 belonged to the round-1 Ising keying and are retired.) */
+enum { DOM_SITE = 0, DOM_INIT = 2, DOM_XYDIR = 3, DOM_GROUP = 5 };
+enum { GROUP_DRAW_BASE = 128, GROUP_WORDS = 160 };
 
 struct swo_ctx {
     int dim, L, model, q;
@@ -70,6 +81,8 @@ struct swo_ctx {
     double forced_phi;
     /* statistics of the last step's bond configuration */
     double n_active, n_clusters, sum_nc2;
+    /* the words W_G[0 .. 32 dim] of the group make_bonds is working on */
+    uint32_t gw[GROUP_WORDS];
 };
 
 static void draw(const swo_ctx *o, uint32_t site, uint64_t t, uint32_t domain, uint32_t w[4])
@@ -168,39 +181,28 @@ static uint32_t threshold32(double p)
     return (uint32_t)v;
 }
 
-/* Ising, reading 6: the random bits of site i at step t.  The 128 output bits of the PACK call
- * number i / S are cut into S pieces of W = 128 / S bits, in word order; site i owns piece i % S
- * (2D: word i % 4; 3D: words 2 (i % 2) [low] and 2 (i % 2) + 1 [high]).  Inside its piece, bond k
- * has the F-bit field at bit offset k F, with F = (W - 1) / dim (15 in 2D, 21 in 3D), and the top
- * bit of the piece is the new value of the cluster whose root is this site. */
-static int ising_field_bits(const swo_ctx *o) { return (o->dim == 2) ? 15 : 21; }
-
-static void ising_site_bits(const swo_ctx *o, size_t i, uint64_t t, uint32_t field[3], int *top_bit)
+/* Reading 6, domain GROUP: word n of the stream of group G at step t. */
+static uint32_t group_word(const swo_ctx *o, uint32_t G, uint64_t t, uint32_t n)
 {
-    const int S = (o->dim == 2) ? 4 : 2;
-    const int W = 128 / S;
-    const int F = ising_field_bits(o);
     uint32_t w[4];
-    draw(o, (uint32_t)(i / (size_t)S), t, DOM_PACK, w);
-    uint64_t piece;
-    if (o->dim == 2) piece = w[i % 4];
-    else piece = (uint64_t)w[2 * (i % 2)] | ((uint64_t)w[2 * (i % 2) + 1] << 32);
-    for (int k = 0; k < o->dim; ++k) field[k] = (uint32_t)((piece >> (F * k)) & ((1u << F) - 1u));
-    *top_bit = (int)((piece >> (W - 1)) & 1u);
+    draw(o, G, t, (uint32_t)DOM_GROUP + 256u * (n >> 2), w);
+    return w[n & 3u];
 }
 
-/* Ising bond decision with probability exactly P32 / 2^32 from an F-bit field: compare the field
- * with the top F bits of P32; only if they are equal (probability 2^-F) the remaining 32 - F bits
- * of P32 are compared with the top 32 - F bits of word k of the site's TIE call. */
-static int ising_bond_random(const swo_ctx *o, size_t i, uint64_t t, int k, uint32_t field, uint32_t P32)
+/* The words W_G[0 .. 32 dim] (draw bits and the 32 binary digits of every bond's uniform integer)
+ * of group G, four per Philox call. */
+static void group_fill(swo_ctx *o, uint32_t G, uint64_t t)
 {
-    const int F = ising_field_bits(o);
-    const uint32_t Ptop = P32 >> (32 - F), Plow = P32 & ((1u << (32 - F)) - 1u);
-    if (field < Ptop) return 1;
-    if (field > Ptop) return 0;
-    uint32_t w[4];
-    draw(o, (uint32_t)i, t, DOM_TIE, w);
-    return (w[k] >> F) < Plow;
+    const uint32_t nwords = 1u + 32u * (uint32_t)o->dim;
+    for (uint32_t c = 0; 4u * c < nwords; ++c) draw(o, G, t, (uint32_t)DOM_GROUP + 256u * c, &o->gw[4u * c]);
+}
+
+/* u(site, k): digit s (bit 31 - s) is bit b of W_G[1 + s dim + k]. */
+static uint32_t group_uniform(const swo_ctx *o, uint32_t b, int k)
+{
+    uint32_t u = 0;
+    for (int s = 0; s < 32; ++s) u |= ((o->gw[1 + s * o->dim + k] >> b) & 1u) << (31 - s);
+    return u;
 }
 
 /* Sub-step (1): active-bond generation. */
@@ -208,31 +210,20 @@ static void make_bonds(swo_ctx *o)
 {
     const uint64_t t = o->t;
     double nact = 0.0;
-    if (o->model == SWO_ISING) {
-        uint32_t P32 = threshold32(-expm1(-2.0 * o->beta));
+    if (o->model == SWO_ISING || o->model == SWO_POTTS) {
+        /* PAPER.md:96 (Ising), PAPER.md:152 + Eq. 2 (Potts): a bond between equal neighbours is active
+         * with probability p; readings 1, 2, 16: active iff u(site, k) < floor(p 2^32). */
+        const uint32_t P32 = threshold32(o->model == SWO_ISING ? -expm1(-2.0 * o->beta) : -expm1(-o->beta));
         for (size_t i = 0; i < o->N; ++i) {
-            uint32_t field[3];
-            int top;
-            ising_site_bits(o, i, t, field, &top);
+            if ((i & 31u) == 0) group_fill(o, (uint32_t)(i >> 5), t);
             uint8_t b = 0;
             for (int k = 0; k < o->dim; ++k) {
                 size_t j = nbr_plus(o, i, k);
-                if (o->s_ising[i] == o->s_ising[j] && ising_bond_random(o, i, t, k, field[k], P32)) {
+                int equal = (o->model == SWO_ISING) ? (o->s_ising[i] == o->s_ising[j]) : (o->s_potts[i] == o->s_potts[j]);
+                if (equal && group_uniform(o, (uint32_t)(i & 31u), k) < P32) {
                     b |= (uint8_t)(1u << k);
                     nact += 1.0;
                 }
-            }
-            o->bond[i] = b;
-        }
-    } else if (o->model == SWO_POTTS) {
-        uint32_t P32 = threshold32(-expm1(-o->beta));
-        for (size_t i = 0; i < o->N; ++i) {
-            uint32_t w[4];
-            draw(o, (uint32_t)i, t, DOM_SITE, w);
-            uint8_t b = 0;
-            for (int k = 0; k < o->dim; ++k) {
-                size_t j = nbr_plus(o, i, k);
-                if (o->s_potts[i] == o->s_potts[j] && w[k] < P32) { b |= (uint8_t)(1u << k); nact += 1.0; }
             }
             o->bond[i] = b;
         }
@@ -340,8 +331,9 @@ static void label_clusters(swo_ctx *o)
 }
 
 /* Sub-step (3): "All spins in each cluster are set randomly to +1 or -1" (reading
- * 5: a fresh value, not "flip with probability 1/2").  One draw per cluster at its root:
- * Ising the top bit of the root's PACK piece, Potts and XY word 3 of the root's SITE call.  Potts: new state (w*q) >> 32.  XY (mirror
+ * 5: a fresh value, not "flip with probability 1/2").  One draw per cluster at its root (reading 6):
+ * Ising the root's bit of W_G[0]; Potts the root's draw word w = W_G[128 + b], new state (w*q) >> 32;
+ * XY and clock the top bit of word 3 of the root's SITE call.  XY (mirror
  * projection): if the top bit is set, reflect every spin of the cluster across the line
  * perpendicular to r: theta' = c - theta with c = (2 phi + pi) mod 2 pi, wrapped to [0, 2 pi]
  * -- two fp32 operations, done in float here exactly as the spec states them. */
@@ -351,14 +343,17 @@ static void flip_clusters(swo_ctx *o)
     const float two_pi_f = (float)TWO_PI;
     for (size_t i = 0; i < o->N; ++i) {
         uint32_t w[4];
+        const uint32_t root = o->label[i];
         if (o->model == SWO_ISING) {
-            uint32_t field[3];
-            int top;
-            ising_site_bits(o, o->label[i], t, field, &top);
-            o->s_ising[i] = top ? 1 : -1;
+            o->s_ising[i] = ((group_word(o, root >> 5, t, 0) >> (root & 31u)) & 1u) ? 1 : -1;
             continue;
         }
-        draw(o, o->label[i], t, DOM_SITE, w);
+        if (o->model == SWO_POTTS) {
+            const uint32_t wd = group_word(o, root >> 5, t, (uint32_t)GROUP_DRAW_BASE + (root & 31u));
+            o->s_potts[i] = (uint8_t)(((uint64_t)wd * (uint64_t)o->q) >> 32);
+            continue;
+        }
+        draw(o, root, t, DOM_SITE, w);
         if (o->model == SWO_CLOCK) {
             /* mirror projection of the whole cluster with probability 1/2: p -> (m - p) mod q */
             if (w[3] >> 31) {
@@ -368,8 +363,7 @@ static void flip_clusters(swo_ctx *o)
             }
             continue;
         }
-        if (o->model == SWO_POTTS) o->s_potts[i] = (uint8_t)(((uint64_t)w[3] * (uint64_t)o->q) >> 32);
-        else if (w[3] >> 31) {
+        if (w[3] >> 31) {
             float th = o->crefl - o->s_xy[i];
             if (th < 0.0f) th = th + two_pi_f;
             o->s_xy[i] = th;

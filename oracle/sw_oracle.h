@@ -10,11 +10,16 @@
  * includes the other.  Readings of the paper (where it is silent or garbled) are listed in
  * DESIGN.md section 3 ("Readings"); each function in sw_oracle.c cites the passage it follows.
  *
- * Parity pins (tests/test_oracle_*.py, all -m "not gpu"): Philox known-answer vectors, exact
- * enumeration of 4x4 / 3x3 Ising and 3x3 q=3 Potts, Kaufman's finite-torus energy, structural
- * invariants checked with an independent union-find, Ising == Potts(q=2) bit identity, XY vs an
- * independent Metropolis sampler.  Nothing in this file is "parity unpinned"; for continuous XY
- * the pin is statistical (no closed form exists).
+ * Parity pins (tests/test_oracle_*.py, all -m "not gpu", statistical ones at 3 sigma): Philox
+ * known-answer vectors, exact enumeration of 4x4 / 3x3 Ising and 3x3 q=3 Potts, Kaufman's
+ * finite-torus energy, structural invariants checked with scipy's connected components, bias /
+ * independence of the transposed bond randoms (reading 6), Ising(beta) and Potts(q=2, 2 beta) giving
+ * the same bonds and clusters from the same configuration and the same moments (the bit identity of
+ * whole trajectories, does not hold: the two models key their cluster draws
+ * differently), XY vs an independent Metropolis sampler, the clock model vs enumeration.
+ * Nothing in this file is "parity unpinned" except init_spins (the seeded start, reading 15): it is
+ * compared with the CUDA path's start state only, which is harmless -- any start state is a valid
+ * input of the chain.  For continuous XY the pin is statistical (no closed form exists).
  */
 #ifndef SW_ORACLE_H
 #define SW_ORACLE_H

@@ -116,5 +116,5 @@ def test_clock_512_matches_continuous_xy():
         res[model] = (np.mean([x[0] for x in es]), np.sqrt(np.sum([x[1] ** 2 for x in es])) / 3,
                       np.mean([x[0] for x in ms]), np.sqrt(np.sum([x[1] ** 2 for x in ms])) / 3)
     c, x = res[so.CLOCK], res[so.XY]
-    assert abs(c[0] - x[0]) <= 3.5 * math.hypot(c[1], x[1]) + 2e-4
-    assert abs(c[2] - x[2]) <= 3.5 * math.hypot(c[3], x[3]) + 2e-4
+    assert abs(c[0] - x[0]) <= 3.0 * math.hypot(c[1], x[1])
+    assert abs(c[2] - x[2]) <= 3.0 * math.hypot(c[3], x[3])

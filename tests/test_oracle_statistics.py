@@ -5,8 +5,8 @@ draw are all right; a dropped factor 2 in beta, a missed wrap bond, a biased dra
 random stream each shift at least one of these averages by many sigma.  Exact values come from
 tests/exact.py (brute-force enumeration / Kaufman's formula, themselves pinned in
 test_exact_pins.py to the numbers SURVEY.md section 8(c) S6 prints).  Fixed seeds, 4 independent
-runs as in the paper; pass = |mean - exact| <= 4 sigma of the pooled binned error
-(4 rather than 3 because ~40 quantities are tested with fixed seeds; none is re-tuned).
+runs as in the paper; pass = |mean - exact| <= 3 sigma of the pooled binned error
+(north_star's tolerance; fixed seeds, none is re-tuned).
 """
 import math
 
@@ -18,7 +18,7 @@ from oracle import sw_oracle as so
 from stats import pooled
 
 SEEDS = (1, 2, 3, 4)
-NSIG = 4.0
+NSIG = 3.0
 
 
 def _runs(dim, L, model, q, beta, nsteps, discard=1000):

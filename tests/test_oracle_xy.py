@@ -16,7 +16,7 @@ from lattice_ref import plus_neighbours
 from oracle import sw_oracle as so
 from stats import binned_mean_err, pooled
 
-NSIG = 4.0
+NSIG = 3.0
 
 
 def test_xy_restricted_to_two_angles_is_the_ising_model():
