@@ -13,7 +13,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsw_b200.so")
 SOURCES = [os.path.join(CSRC, "sw_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "sw_kernels.cuh"), os.path.join(ROOT, "include", "sw.h")]
+DEPS = SOURCES + [os.path.join(CSRC, "sw_kernels.cuh"), os.path.join(CSRC, "sw_rows.cuh"), os.path.join(ROOT, "include", "sw.h")]
 
 
 def nvcc_path() -> str:

@@ -4,6 +4,7 @@
 // any lattice size); no host synchronisation inside sw_step.
 #include "../../include/sw.h"
 #include "sw_kernels.cuh"
+#include "sw_rows.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -27,7 +28,7 @@ int fail(int code, const std::string &msg)
 
 // One tile configuration = the tiled kernels instantiated for it.
 struct TileOps {
-    int tx, ty, tz, nt, qpt, nfw, log2ns;
+    int tx, ty, tz, nt, nt_bl, rows;   // nt: threads of k_flip, nt_bl: threads of the bond / label kernel
     size_t smem_bond_label;
     void (*bond_label)(const Params);
     void (*merge)(const Params);
@@ -36,6 +37,7 @@ struct TileOps {
     void (*tile_origin)(const Params);
 };
 
+// XY, clock: k_bond_label (a thread owns QPT quads of 4 sites).
 template <int DIM, int MODEL, int TX, int TY, int TZ, int QPT = 4>
 TileOps make_ops()
 {
@@ -43,7 +45,7 @@ TileOps make_ops()
     constexpr int NS = G::NS;
     constexpr int NT = NS / (4 * QPT);  // QPT quads = 4 QPT sites per thread
     TileOps o;
-    o.tx = TX; o.ty = TY; o.tz = TZ; o.nt = NT; o.qpt = QPT; o.nfw = G::NFW; o.log2ns = G::LOG2NS;
+    o.tx = TX; o.ty = TY; o.tz = TZ; o.nt = NT; o.nt_bl = NT; o.rows = 0;
     o.smem_bond_label = G::template smem_bond_label<MODEL>();
     o.bond_label = k_bond_label<DIM, MODEL, TX, TY, TZ, NT>;
     o.merge = k_merge<DIM, TX, TY, TZ>;
@@ -53,7 +55,51 @@ TileOps make_ops()
     return o;
 }
 
-// Tile menu.  Tile sides are powers of two, TX in {32, 64, 128}; every side must divide L.
+// Ising, Potts: k_bond_label_rows (a thread owns R rows of 32 sites); k_flip with QPT quads per thread.
+template <int DIM, int MODEL, int TY, int TZ, int R, int QPT, int MINB>
+TileOps make_ops_rows()
+{
+    using G = RowGeom<DIM, MODEL, TY, TZ>;
+    constexpr int NT = G::NS / (4 * QPT);
+    TileOps o;
+    o.tx = 32; o.ty = TY; o.tz = TZ; o.nt = NT; o.nt_bl = RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT; o.rows = R;
+    o.smem_bond_label = G::smem_bytes;
+    o.bond_label = k_bond_label_rows<DIM, MODEL, TY, TZ, R, MINB>;
+    o.merge = k_merge<DIM, 32, TY, TZ>;
+    o.flip = k_flip<DIM, MODEL, 32, TY, TZ, NT>;
+    o.export_labels = k_export_labels<DIM, 32, TY, TZ>;
+    o.tile_origin = k_tile_origin<32, TY, TZ>;
+    return o;
+}
+
+// Tile menu of the row kernel (Ising, Potts): 32 x TY (x TZ) sites, R rows per thread.  rows = 0 picks the
+// default R of the tile.
+template <int MODEL>
+bool pick_ops_rows(int dim, int tx, int ty, int tz, int rows, TileOps &o)
+{
+    if (tx != 32) return false;
+#define SW_ROWS2(Y, RR, Q, B) if (dim == 2 && ty == Y && (rows == RR || rows == 0)) { o = make_ops_rows<2, MODEL, Y, 1, RR, Q, B>(); return true; }
+#define SW_ROWS3(Z, RR, Q, B) if (dim == 3 && ty == 32 && tz == Z && (rows == RR || rows == 0)) { o = make_ops_rows<3, MODEL, 32, Z, RR, Q, B>(); return true; }
+    SW_ROWS2(32, 1, 1, 16)
+    SW_ROWS2(128, 2, 4, 8)
+    SW_ROWS2(128, 1, 4, 8)
+    SW_ROWS2(256, 2, 4, 6)
+    SW_ROWS2(256, 4, 4, 6)
+    SW_ROWS2(512, 4, 8, 3)
+    SW_ROWS2(512, 2, 8, 3)
+    SW_ROWS3(4, 1, 4, 8)
+    SW_ROWS3(8, 2, 4, 6)
+    SW_ROWS3(8, 1, 4, 6)
+    SW_ROWS3(16, 2, 8, 3)
+    SW_ROWS3(16, 4, 8, 3)
+    SW_ROWS3(16, 1, 8, 3)
+#undef SW_ROWS2
+#undef SW_ROWS3
+    return false;
+}
+
+// Tile menu of the quad kernel (XY, clock).  Tile sides are powers of two, TX in {32, 64, 128}; every side
+// must divide L.
 template <int MODEL>
 bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
 {
@@ -67,56 +113,43 @@ bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
     SW_TILE3(32, 16, 8)
     SW_TILE3(32, 16, 16)
     SW_TILE3(64, 8, 8)
-    if (dim == 3 && tx == 32 && ty == 32 && tz == 16) { o = make_ops<3, MODEL, 32, 32, 16, 8>(); return true; }  // 8 quads per thread
 #undef SW_TILE2
 #undef SW_TILE3
     return false;
 }
 
 // Small lattices (fewer tiles than the GPU has room for): what counts is the critical path of one CTA,
-// so the smallest tile of the menu with ONE quad per thread (4x the threads for the same tile).
-template <int MODEL>
-bool pick_ops_small(int dim, TileOps &o)
+// so the smallest tile of the menu with the fewest sites per thread.
+bool pick_ops_small_model(int model, int dim, TileOps &o)
 {
-    if (dim == 2) o = make_ops<2, MODEL, 32, 32, 1, 1>(); else o = make_ops<3, MODEL, 32, 8, 8, 1>();
+    if (model == SW_ISING) return pick_ops_rows<ISING>(dim, 32, 32, dim == 3 ? 4 : 1, 1, o);
+    if (model == SW_POTTS) return pick_ops_rows<POTTS>(dim, 32, 32, dim == 3 ? 4 : 1, 1, o);
+    if (model == SW_CLOCK) { if (dim == 2) o = make_ops<2, CLOCK, 32, 32, 1, 1>(); else o = make_ops<3, CLOCK, 32, 8, 8, 1>(); return true; }
+    if (dim == 2) o = make_ops<2, XY, 32, 32, 1, 1>(); else o = make_ops<3, XY, 32, 8, 8, 1>();
     return true;
 }
 
-bool pick_ops_small_model(int model, int dim, TileOps &o)
+bool pick_ops_model(int model, int dim, int tx, int ty, int tz, int rows, TileOps &o)
 {
-#ifdef SW_MENU_MIN
-    return false;
-#endif
-    if (model == SW_ISING) return pick_ops_small<ISING>(dim, o);
-    if (model == SW_POTTS) return pick_ops_small<POTTS>(dim, o);
-    if (model == SW_CLOCK) return pick_ops_small<CLOCK>(dim, o);
-    return pick_ops_small<XY>(dim, o);
-}
-
-bool pick_ops_model(int model, int dim, int tx, int ty, int tz, TileOps &o)
-{
-#ifdef SW_MENU_MIN  // developer builds: one model, one tile per dimension (fast to compile)
-    if (dim == 3) o = make_ops<3, ISING, 32, 16, 16>(); else o = make_ops<2, ISING, 128, 64, 1>();
-    return model == SW_ISING && tx == o.tx && ty == o.ty && tz == o.tz;
-#endif
-    if (model == SW_ISING) return pick_ops<ISING>(dim, tx, ty, tz, o);
-    if (model == SW_POTTS) return pick_ops<POTTS>(dim, tx, ty, tz, o);
+    if (model == SW_ISING) return pick_ops_rows<ISING>(dim, tx, ty, tz, rows, o);
+    if (model == SW_POTTS) return pick_ops_rows<POTTS>(dim, tx, ty, tz, rows, o);
     if (model == SW_CLOCK) return pick_ops<CLOCK>(dim, tx, ty, tz, o);
     return pick_ops<XY>(dim, tx, ty, tz, o);
 }
 
-// Default tile of a lattice (SW_B200_TILE=TXxTYxTZ overrides it: a tuning knob).
+// Default tile of a lattice (SW_B200_TILE=TXxTYxTZ and SW_B200_ROWS=R override it: tuning knobs).
 void default_tile(int dim, int L, int model, int &tx, int &ty, int &tz)
 {
+    const bool rows = model == SW_ISING || model == SW_POTTS;
     if (dim == 2) {
         tz = 1;
-        if (L % 64 == 0) { tx = 64; ty = 64; }   // measured on C2 / C3: 64x64 3 % ahead of 128x64
+        if (rows) { tx = 32; ty = (L % 256 == 0) ? 256 : (L % 128 == 0 ? 128 : 32); }
+        else if (L % 64 == 0) { tx = 64; ty = 64; }   // measured on C2 / C3 (round 1): 64x64 3 % ahead of 128x64
         else { tx = 32; ty = 32; }
     } else {
-        tx = 32; ty = 16; tz = 16;  // also for XY (75 KB of shared memory per CTA: projections + labels)
-        // Ising on very large lattices: 32x32x16 tiles with 8 quads per thread -- a fifth fewer bonds
-        // through tile faces, measured 2 % ahead at L = 512 (behind at L = 256 and for the other models)
-        if (model == SW_ISING && (double)L * L * L >= 134217728.0) ty = 32;
+        tx = 32;
+        if (rows) { ty = 32; tz = (L % 16 == 0) ? 16 : (L % 8 == 0 ? 8 : 4); }
+        else { ty = 16; tz = 16; }  // XY: 75 KB of shared memory per CTA (projections + labels)
     }
 }
 
@@ -340,7 +373,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     if (!out) return fail(SW_EINVAL, "out is NULL");
     *out = nullptr;
     if (!valid_args(dim, L, model, q, beta, true))
-        return fail(SW_EINVAL, "invalid arguments (dim 2|3, L multiple of 32 with L^dim <= 2^31 and L^dim 2^ceil(log2 q) <= 2^32, model, 2<=q<=255, beta>=0)");
+        return fail(SW_EINVAL, "invalid arguments (dim 2|3, L multiple of 32 with L^dim <= 2^31 and L^dim 2^ceil(log2 q) <= 2^32, model, Potts 2<=q<=255 / clock 2<=q<=512, beta>=0)");
     const Layout lay = layout(dim, L, model, q);
     if (external) {
         if (!workspace || workspace_bytes < lay.total || ((uintptr_t)workspace & 255u))
@@ -367,21 +400,20 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
         e = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking);
         if (e != cudaSuccess) { cudaFree(c->workspace); delete c; return fail(SW_ECUDA, "cudaStreamCreate failed"); }
     }
-    // tile choice: default per dimension and model, SW_B200_TILE=TXxTYxTZ overrides (tuning knob)
-    int tx, ty, tz;
+    // tile choice: default per dimension and model, SW_B200_TILE=TXxTYxTZ / SW_B200_ROWS=R override (tuning knobs)
+    int tx, ty, tz, rows = 0;
     default_tile(dim, L, model, tx, ty, tz);
-    if (const char *env = std::getenv("SW_B200_TILE")) {
+    const char *env_tile = std::getenv("SW_B200_TILE");
+    if (env_tile) {
         int ex = 0, ey = 0, ez = 1;
-        if (std::sscanf(env, "%dx%dx%d", &ex, &ey, &ez) >= 2) { tx = ex; ty = ey; tz = (dim == 2) ? 1 : ez; }
+        if (std::sscanf(env_tile, "%dx%dx%d", &ex, &ey, &ez) >= 2) { tx = ex; ty = ey; tz = (dim == 2) ? 1 : ez; }
     }
+    if (const char *env = std::getenv("SW_B200_ROWS")) rows = std::atoi(env);
     bool ok = tx > 0 && ty > 0 && tz > 0 && (L % tx == 0) && (L % ty == 0) && (L % tz == 0) &&
-              pick_ops_model(model, dim, tx, ty, tz, c->ops);
-    if (!ok) {
-        tx = 32; ty = (dim == 2) ? 32 : 8; tz = (dim == 2) ? 1 : 8;
-        pick_ops_model(model, dim, tx, ty, tz, c->ops);
-    }
-    if (!std::getenv("SW_B200_TILE")) {
-        // fewer default tiles than 2 per SM: latency variant (smallest tile, one quad per thread)
+              pick_ops_model(model, dim, tx, ty, tz, rows, c->ops);
+    if (!ok) ok = pick_ops_small_model(model, dim, c->ops);
+    if (!env_tile) {
+        // fewer default tiles than 2 per SM: latency variant (smallest tile, fewest sites per thread)
         int sms = 148, dev = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -516,7 +548,7 @@ int build_graph(sw_ctx *c, int steps, cudaGraphExec_t *out)
             cudaKernelNodeParams kp = {};
             kp.kernelParams = args;
             kp.extra = nullptr;
-            if (k == 0) { kp.func = (void *)c->ops.bond_label; kp.gridDim = grid; kp.blockDim = dim3(c->ops.nt); kp.sharedMemBytes = (unsigned)c->ops.smem_bond_label; }
+            if (k == 0) { kp.func = (void *)c->ops.bond_label; kp.gridDim = grid; kp.blockDim = dim3(c->ops.nt_bl); kp.sharedMemBytes = (unsigned)c->ops.smem_bond_label; }
             if (k == 1) { kp.func = (void *)c->ops.merge; kp.gridDim = dim3(c->merge_blocks); kp.blockDim = dim3(256); kp.sharedMemBytes = 0; }
             if (k == 2) { kp.func = (void *)c->ops.flip; kp.gridDim = grid; kp.blockDim = dim3(c->ops.nt); kp.sharedMemBytes = 0; }
             cudaGraphNode_t node = nullptr;
@@ -585,7 +617,7 @@ int sw_step(sw_ctx *c, int n)
             SW_CUDA(c, cudaMemcpyAsync(&p.acc->stats[0], &examined, 8, cudaMemcpyHostToDevice, c->stream));
         }
         if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[0], c->stream));
-        c->ops.bond_label<<<grid, c->ops.nt, c->ops.smem_bond_label, c->stream>>>(p);
+        c->ops.bond_label<<<grid, c->ops.nt_bl, c->ops.smem_bond_label, c->stream>>>(p);
         if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[1], c->stream));
         c->ops.merge<<<c->merge_blocks, 256, 0, c->stream>>>(p);
         if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[2], c->stream));

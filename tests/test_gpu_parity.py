@@ -63,8 +63,8 @@ def test_philox_device_known_answers():
     (3, 32, 1, 20, 1.2, 20),       # q > 8: shared-memory histogram path
     (2, 160, 0, 0, TC2, 12),       # tile sides that are not the default (L % 128 != 0, L % 64 != 0)
     (2, 224, 1, 17, 0.9, 8),
-    (2, 2048, 0, 0, TC2, 3),       # default large-lattice tiling in 2D (128 x 64, four quads per thread)
-    (3, 160, 0, 0, T3, 3),         # default large-lattice tiling in 3D (32 x 16 x 16), L not a power of two
+    (2, 2048, 0, 0, TC2, 3),       # default large-lattice tiling in 2D
+    (3, 160, 0, 0, T3, 3),         # default large-lattice tiling in 3D, L not a power of two
     (3, 96, 1, 2, 1.1, 5),
     (2, 64, 1, 255, 0.6, 10),      # largest q
 ])
@@ -83,28 +83,65 @@ def test_full_trajectory_bit_exact(dim, L, model, q, T, steps):
     assert (e, m, m2, m4) == pytest.approx(o.observables(), rel=1e-14)
 
 
-@pytest.mark.parametrize("tile", ["32x32", "64x64", "128x32", "128x64"])
-def test_tile_menu_2d(tile, monkeypatch):
-    sw, orc = _mods()
-    monkeypatch.setenv("SW_B200_TILE", tile)
-    g = sw.SwendsenWang(2, 256, 0, 0, 1.0 / TC2, seed=5, record_bonds=True)
-    o = orc.Oracle(2, 256, 0, 0, 1.0 / TC2, 5)
-    for t in range(25):
-        g.step(1)
-        o.step(1)
-        _compare_step(g, o, f"tile {tile} t={t}")
+# Tile menus.  Ising / Potts run the row kernel (tiles 32 x TY (x TZ), R rows per thread: SW_B200_TILE,
+# SW_B200_ROWS), XY / clock the quad kernel; small lattices would silently take the smallest tile, so every
+# instantiation bench.py can time is forced here by name.
+ROW_TILES_2D = [("32x32", 1), ("32x128", 1), ("32x128", 2), ("32x256", 2), ("32x256", 4), ("32x512", 2), ("32x512", 4)]
+ROW_TILES_3D = [("32x32x4", 1), ("32x32x8", 1), ("32x32x8", 2), ("32x32x16", 1), ("32x32x16", 2), ("32x32x16", 4)]
 
 
-@pytest.mark.parametrize("tile", ["32x8x8", "32x16x8", "32x16x16", "64x8x8", "32x32x16"])
-def test_tile_menu_3d(tile, monkeypatch):
+@pytest.mark.parametrize("model,q,T", [(0, 0, TC2), (1, 3, TP3), (1, 9, 0.8)])
+@pytest.mark.parametrize("tile,rows", ROW_TILES_2D)
+def test_tile_menu_2d(tile, rows, model, q, T, monkeypatch):
     sw, orc = _mods()
     monkeypatch.setenv("SW_B200_TILE", tile)
-    g = sw.SwendsenWang(3, 64, 0, 0, 1.0 / T3, seed=5, record_bonds=True)
-    o = orc.Oracle(3, 64, 0, 0, 1.0 / T3, 5)
+    monkeypatch.setenv("SW_B200_ROWS", str(rows))
+    g = sw.SwendsenWang(2, 512, model, q, 1.0 / T, seed=5, record_bonds=True)
+    o = orc.Oracle(2, 512, model, q, 1.0 / T, 5)
     for t in range(12):
         g.step(1)
         o.step(1)
-        _compare_step(g, o, f"tile {tile} t={t}")
+        _compare_step(g, o, f"tile {tile} R={rows} model {model} t={t}")
+
+
+@pytest.mark.parametrize("model,q,T", [(0, 0, T3), (1, 3, 1.8), (1, 20, 1.2)])
+@pytest.mark.parametrize("tile,rows", ROW_TILES_3D)
+def test_tile_menu_3d(tile, rows, model, q, T, monkeypatch):
+    sw, orc = _mods()
+    monkeypatch.setenv("SW_B200_TILE", tile)
+    monkeypatch.setenv("SW_B200_ROWS", str(rows))
+    g = sw.SwendsenWang(3, 64, model, q, 1.0 / T, seed=5, record_bonds=True)
+    o = orc.Oracle(3, 64, model, q, 1.0 / T, 5)
+    for t in range(8):
+        g.step(1)
+        o.step(1)
+        _compare_step(g, o, f"tile {tile} R={rows} model {model} t={t}")
+
+
+@pytest.mark.parametrize("dim,L,tile", [(2, 256, "32x32"), (2, 256, "64x64"), (2, 256, "128x32"), (2, 256, "128x64"),
+                                        (3, 64, "32x8x8"), (3, 64, "32x16x8"), (3, 64, "32x16x16"), (3, 64, "64x8x8")])
+@pytest.mark.parametrize("model,q", [(2, 0), (3, 12)])
+def test_tile_menu_xy_clock(dim, L, tile, model, q, monkeypatch):
+    """The quad kernel's tiles for the two models that use it: XY (bond mismatch budget) and clock (bit-exact)."""
+    sw, orc = _mods()
+    monkeypatch.setenv("SW_B200_TILE", tile)
+    T = 0.9 if dim == 2 else 2.2019
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=5, record_bonds=True)
+    o = orc.Oracle(dim, L, model, q, 1.0 / T, 5)
+    bad = 0
+    for t in range(6):
+        if model == 2:
+            o.set_spins(g.spins(), g.t)
+        g.step(1)
+        o.step(1)
+        if model == 3:
+            _compare_clock_step(g, o, f"tile {tile} clock t={t}")
+        else:
+            nb = int(np.count_nonzero(g.bonds() != o.bonds()))
+            bad += nb
+            if nb == 0:
+                assert np.array_equal(g.labels(), o.labels()) and np.array_equal(g.spins(), o.spins())
+    assert bad <= 1
 
 
 @pytest.mark.parametrize("dim,L,model,q", [(2, 128, 0, 0), (3, 32, 0, 0), (2, 128, 1, 3)])
@@ -184,32 +221,6 @@ def test_determinism_and_step_batching():
     c = sw.SwendsenWang(2, 256, 0, 0, 1.0 / TC2, seed=10)
     c.step(5)
     assert not np.array_equal(a.spins(), c.spins())
-
-
-@pytest.mark.parametrize("dim,L", [(2, 64), (3, 32)])
-def test_ising_forced_tie_parity(dim, L):
-    """Packed Ising keying (reading 6): a bond whose F-bit field equals the top F bits of
-    the threshold is settled by the TIE call.  That has probability 2^-F per bond, so the case is
-    forced: beta is chosen so that the threshold's top part equals a field that does occur."""
-    sw, orc = _mods()
-    from paper_1403_7560_b200 import inputs
-    seed, t0, N = 21, 7, L ** dim
-    S, W = (4, 32) if dim == 2 else (2, 64)
-    F = (W - 1) // dim
-    for site, k in [(3, 0), (N // 3, dim - 1), (N - 2, 1)]:
-        w = orc.philox4x32_10([site // S, t0, 0, 1], [seed, 0])
-        piece = w[site % 4] if dim == 2 else (w[2 * (site % 2)] | (w[2 * (site % 2) + 1] << 32))
-        v = (piece >> (F * k)) & ((1 << F) - 1)
-        beta = -0.5 * math.log1p(-(v + 0.5) / (1 << F))
-        g = sw.SwendsenWang(dim, L, 0, 0, beta, seed=seed, record_bonds=True)
-        o = orc.Oracle(dim, L, 0, 0, beta, seed)
-        cold = inputs.aligned_spins(0, N)
-        g.set_spins(cold, t0)
-        o.set_spins(cold, t0)
-        g.step(1)
-        o.step(1)
-        _compare_step(g, o, f"forced tie dim{dim} site {site} dir {k}")
-        g.close()
 
 
 def test_state_errors():
