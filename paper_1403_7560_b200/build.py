@@ -13,7 +13,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsw_b200.so")
 SOURCES = [os.path.join(CSRC, "sw_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "sw_kernels.cuh"), os.path.join(CSRC, "sw_rows.cuh"), os.path.join(ROOT, "include", "sw.h")]
+DEPS = SOURCES + [os.path.join(CSRC, "sw_kernels.cuh"), os.path.join(CSRC, "sw_rows.cuh"), os.path.join(CSRC, "sw_small.cuh"), os.path.join(ROOT, "include", "sw.h")]
 
 
 def nvcc_path() -> str:
@@ -30,6 +30,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
            "-Xcompiler", "-fPIC", "-shared", "-o", LIB] + SOURCES
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
+    cmd[1:1] = os.environ.get("SW_B200_NVCC_FLAGS", "").split()   # developer knob: extra -D... for experiments
     subprocess.run(cmd, check=True)
     return LIB
 

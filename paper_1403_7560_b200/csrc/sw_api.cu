@@ -5,6 +5,7 @@
 #include "../../include/sw.h"
 #include "sw_kernels.cuh"
 #include "sw_rows.cuh"
+#include "sw_small.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -78,6 +79,12 @@ template <int MODEL>
 bool pick_ops_rows(int dim, int tx, int ty, int tz, int rows, TileOps &o)
 {
     if (tx != 32) return false;
+#ifdef SW_MENU_MIN   // developer builds: few instantiations (fast to compile)
+    if (MODEL != ISING) return false;
+    if (dim == 3 && ty == 32 && tz == 16) { o = make_ops_rows<3, ISING, 32, 16, 1, 8, 3>(); return true; }
+    if (dim == 2 && ty == 256) { o = make_ops_rows<2, ISING, 256, 1, 2, 4, 6>(); return true; }
+    return false;
+#else
 #define SW_ROWS2(Y, RR, Q, B) if (dim == 2 && ty == Y && (rows == RR || rows == 0)) { o = make_ops_rows<2, MODEL, Y, 1, RR, Q, B>(); return true; }
 #define SW_ROWS3(Z, RR, Q, B) if (dim == 3 && ty == 32 && tz == Z && (rows == RR || rows == 0)) { o = make_ops_rows<3, MODEL, 32, Z, RR, Q, B>(); return true; }
     SW_ROWS2(32, 1, 1, 16)
@@ -96,6 +103,7 @@ bool pick_ops_rows(int dim, int tx, int ty, int tz, int rows, TileOps &o)
 #undef SW_ROWS2
 #undef SW_ROWS3
     return false;
+#endif
 }
 
 // Tile menu of the quad kernel (XY, clock).  Tile sides are powers of two, TX in {32, 64, 128}; every side
@@ -103,6 +111,9 @@ bool pick_ops_rows(int dim, int tx, int ty, int tz, int rows, TileOps &o)
 template <int MODEL>
 bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
 {
+#ifdef SW_MENU_MIN
+    return false;
+#endif
 #define SW_TILE2(X, Y) if (dim == 2 && tx == X && ty == Y) { o = make_ops<2, MODEL, X, Y, 1>(); return true; }
 #define SW_TILE3(X, Y, Z) if (dim == 3 && tx == X && ty == Y && tz == Z) { o = make_ops<3, MODEL, X, Y, Z>(); return true; }
     SW_TILE2(32, 32)
@@ -122,6 +133,9 @@ bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
 // so the smallest tile of the menu with the fewest sites per thread.
 bool pick_ops_small_model(int model, int dim, TileOps &o)
 {
+#ifdef SW_MENU_MIN
+    return false;
+#endif
     if (model == SW_ISING) return pick_ops_rows<ISING>(dim, 32, 32, dim == 3 ? 4 : 1, 1, o);
     if (model == SW_POTTS) return pick_ops_rows<POTTS>(dim, 32, 32, dim == 3 ? 4 : 1, 1, o);
     if (model == SW_CLOCK) { if (dim == 2) o = make_ops<2, CLOCK, 32, 32, 1, 1>(); else o = make_ops<3, CLOCK, 32, 8, 8, 1>(); return true; }
@@ -192,9 +206,9 @@ Layout layout(int dim, int L, int model, int q)
     l.bonds = off; off += align256(N);
     l.labels = off; off += align256(N * 4);
     // pair list: one (i, j) address pair per bond through a tile face, sized for the tile of the menu
-    // with the largest face area (3D 32x8x8: (1/32 + 1/8 + 1/8) N bonds; 2D 32x32: N/16); then the
+    // with the largest face area (3D 32x32x4: (1/32 + 1/32 + 1/4) N bonds; 2D 32x32: N/16); then the
     // tile origins (smallest tile: 1024 sites)
-    l.pairs = off; off += align256((dim == 3 ? N / 32 * 9 : N / 16) * 8);
+    l.pairs = off; off += align256((dim == 3 ? N / 32 * 10 : N / 16) * 8);
     l.origin = off; off += align256((N / 1024) * 4);
     l.table = off; off += align256(model == SW_CLOCK ? (size_t)q * q * 4 : 0);  // clock: bond thresholds
     l.acc = off; off += align256(sizeof(Acc));
@@ -215,6 +229,10 @@ struct sw_ctx {
     void *workspace;
     uint8_t *bonds_mem;
     unsigned merge_blocks;
+    // lattices of at most 32768 sites (Ising, Potts): the whole step in one CTA, n steps per launch (sw_small.cuh)
+    bool small;
+    size_t small_smem;
+    void (*small_kernel)(const Params, const SmallArgs);
     // CUDA graphs of 1 and GRAPH_STEPS consecutive steps (3 kernel nodes per step); built lazily for
     // Ising / Potts, rebuilt when the bond-recording flag changes.  XY passes a new direction with
     // every step and keeps plain launches.
@@ -420,6 +438,19 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
         const size_t ntiles_default = c->N / ((size_t)c->ops.tx * c->ops.ty * c->ops.tz);
         if (ntiles_default < (size_t)2 * sms) pick_ops_small_model(model, dim, c->ops);
     }
+    c->small = false; c->small_smem = 0; c->small_kernel = nullptr;
+#ifndef SW_MENU_MIN
+    if ((model == SW_ISING || model == SW_POTTS) && c->N <= 32768 && !std::getenv("SW_B200_NO_SMALL")) {
+        c->small = true;
+        if (model == SW_ISING) {
+            c->small_kernel = (dim == 2) ? k_sw_small<2, ISING> : k_sw_small<3, ISING>;
+            c->small_smem = 4 * ((dim == 2) ? SmallGeom<2, ISING>::words(c->N) : SmallGeom<3, ISING>::words(c->N));
+        } else {
+            c->small_kernel = (dim == 2) ? k_sw_small<2, POTTS> : k_sw_small<3, POTTS>;
+            c->small_smem = 4 * ((dim == 2) ? SmallGeom<2, POTTS>::words(c->N) : SmallGeom<3, POTTS>::words(c->N));
+        }
+    }
+#endif
     char *base = (char *)c->workspace;
     Params &p = c->p;
     p.spins = base + lay.spins;
@@ -475,6 +506,10 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     };
     e = cudaFuncSetAttribute(c->ops.bond_label, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ops.smem_bond_label);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_bond_label)");
+    if (c->small) {
+        e = cudaFuncSetAttribute(c->small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->small_smem);
+        if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_sw_small)");
+    }
     c->ops.tile_origin<<<(p.ntiles + 255) / 256, 256, 0, c->stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return bail(e, "k_tile_origin launch");
@@ -570,6 +605,29 @@ int sw_step(sw_ctx *c, int n)
     if (rc) return rc;
     if (n < 0) return fail(SW_EINVAL, "n < 0");
     const dim3 grid = tile_grid(c);
+    if (c->small) {
+        // one CTA holds the lattice: n steps in one launch
+        if (n == 0) return SW_OK;
+        c->p.bonds = c->record_bonds ? c->bonds_mem : nullptr;
+        SmallArgs a;
+        a.nsteps = n; a.write_labels = 1; a.series = nullptr; a.series_words = 0;
+        if (c->p.counting) SW_CUDA(c, cudaMemsetAsync(c->p.acc->stats, 0, sizeof(c->p.acc->stats), c->stream));
+        if (c->timing) SW_CUDA(c, cudaEventRecord(c->ev[0], c->stream));
+        c->small_kernel<<<1, 1024, c->small_smem, c->stream>>>(c->p, a);
+        if (c->timing) {
+            SW_CUDA(c, cudaEventRecord(c->ev[1], c->stream));
+            SW_CUDA(c, cudaEventSynchronize(c->ev[1]));
+            float ms = 0.f;
+            SW_CUDA(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]));
+            c->kernel_ms[0] += (double)ms;
+            c->timed_steps += (uint64_t)n;
+        }
+        SW_CUDA(c, cudaGetLastError());
+        c->t += (uint64_t)n;
+        c->stepped = true; c->bonds_valid = c->record_bonds != 0;
+        c->M_fresh = true; c->E_fresh = true;   // the kernel leaves E and M of the new configuration in acc
+        return SW_OK;
+    }
     if (c->model != SW_XY && c->model != SW_CLOCK && !c->timing && !c->p.counting && n > 0 && !std::getenv("SW_B200_NO_GRAPH")) {
         // launch-bound regime (small lattices): 3 launches per step cost more host time than the
         // kernels take; replay pre-built graphs instead
@@ -682,7 +740,18 @@ int sw_run_series(sw_ctx *c, int n, double *E, double *M, double *M2, double *M4
         c->series_cap = (size_t)n * words;
     }
     unsigned long long *dser = c->series_dev;
-    for (int s = 0; s < n && rc == SW_OK; ++s) {
+    if (c->small) {
+        // the one-CTA kernel records E and M (n_k) of every step itself
+        c->p.bonds = c->record_bonds ? c->bonds_mem : nullptr;
+        SmallArgs a;
+        a.nsteps = n; a.write_labels = 1; a.series = dser; a.series_words = words;
+        c->small_kernel<<<1, 1024, c->small_smem, c->stream>>>(c->p, a);
+        if (cudaGetLastError() != cudaSuccess) rc = fail(SW_ECUDA, "k_sw_small launch");
+        c->t += (uint64_t)n;
+        c->stepped = true; c->bonds_valid = c->record_bonds != 0;
+        c->M_fresh = true; c->E_fresh = true;
+    }
+    for (int s = 0; s < n && rc == SW_OK && !c->small; ++s) {
         rc = sw_step(c, 1);
         if (rc == SW_OK) rc = refresh_observables(c);
         if (rc == SW_OK) {
@@ -786,7 +855,8 @@ int sw_get_labels(sw_ctx *c, uint32_t *dst, size_t bytes)
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SW_ENOMEM, "sw_get_labels: cudaMalloc of the export buffer failed"); }
     Params q = c->p;
     q.labels_out = out;
-    c->ops.export_labels<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(q);
+    if (c->small) k_export_labels_linear<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(q);
+    else c->ops.export_labels<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(q);
     e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(dst, out, c->N * 4, cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);

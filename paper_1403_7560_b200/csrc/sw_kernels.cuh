@@ -29,7 +29,7 @@
 namespace swk {
 
 enum { ISING = 0, POTTS = 1, XY = 2, CLOCK = 3 };
-constexpr uint32_t DOM_SITE = 0u, DOM_PACK = 1u, DOM_INIT = 2u, DOM_XYDIR = 3u, DOM_TIE = 4u;
+constexpr uint32_t DOM_SITE = 0u, DOM_INIT = 2u, DOM_XYDIR = 3u, DOM_GROUP = 5u;  // DESIGN.md reading 6
 constexpr uint32_t FULL = 0xffffffffu;
 #ifndef SW_BL_THREADS_PER_SM
 #define SW_BL_THREADS_PER_SM 1536  // resident threads per SM k_bond_label is compiled for (register cap)
@@ -226,6 +226,7 @@ __global__ void __launch_bounds__(256) k_tile_origin(const Params p)
 template <int DIM, int MODEL, int TX, int TY, int TZ, int NT>
 __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(const Params p)
 {
+    static_assert(MODEL == XY || MODEL == CLOCK, "Ising and Potts run k_bond_label_rows (sw_rows.cuh)");
     using G = TileGeom<DIM, TX, TY, TZ>;
     constexpr int NS = G::NS, NQ = NS / 4, QPT = NQ / NT, LPR = TX / 4;
     static_assert(NQ % NT == 0 && NT % 32 == 0, "whole quads per thread, whole rows per warp");
@@ -290,12 +291,11 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
     }
     __syncthreads();
 
-    uint32_t bnd[QPT];   // per quad: bits 0-3 x bonds, 4-7 y bonds, 8-11 z bonds
-    uint32_t drw[QPT];   // per quad: the four draws, DB bits each (site s at bit s * db)
+    uint32_t bnd[QPT];   // per quad: bits 0-3 x bonds, 4-7 y bonds, 8-11 z bonds, 12-15 the four 1-bit draws
     // pending bonds that stay inside the tile: bit 4 j + s = site s of the thread's quad j, one mask for
     // the y bonds and one for the z bonds (32-bit masks, and the neighbour offset is a constant per mask)
     uint32_t work[2] = {0u, 0u};
-    const int db = (MODEL == POTTS) ? p.db : 1;
+    constexpr int db = 1;
 
 #pragma unroll
     for (int j = 0; j < QPT; ++j) {
@@ -305,10 +305,8 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
         const uint32_t g = gx + L * (gy + L * gz);
         const bool rowend = (lane & (LPR - 1)) == LPR - 1;
         uint4 w[4];
-        if (MODEL != ISING) {
 #pragma unroll
-            for (int s = 0; s < 4; ++s) w[s] = philox4x32_10(g + s, t_lo, t_hi, DOM_SITE, p.k0, p.k1);
-        }
+        for (int s = 0; s < 4; ++s) w[s] = philox4x32_10(g + s, t_lo, t_hi, DOM_SITE, p.k0, p.k1);
         uint32_t bxn, byn, bzn = 0u, d;
         if (MODEL == XY) {
             // Wolff embedding: aligned iff a_i a_j > 0, p = 1 - exp(-2 beta a_i a_j)
@@ -375,97 +373,9 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
                 if (DIM == 3) bzn |= bond(c0[s], cz[s], w[s].z) << s;
             }
             d = (w[0].w >> 31) | ((w[1].w >> 31) << 1) | ((w[2].w >> 31) << 2) | ((w[3].w >> 31) << 3);
-        } else {
-            // a bond between equal neighbours is active with probability p.
-            const uint8_t *sp = (const uint8_t *)p.spins;
-            const uint32_t own = *reinterpret_cast<const uint32_t *>(sp + g);
-            const uint32_t up = *reinterpret_cast<const uint32_t *>(sp + ((gy + 1 == L) ? g - L * (L - 1) : g + L));
-            uint32_t nb = __shfl_down_sync(FULL, own, 1);
-            if (rowend) nb = sp[(gx + 4 == L) ? g + 4 - L : g + 4];
-            uint32_t fr = 0u;
-            if (DIM == 3) fr = *reinterpret_cast<const uint32_t *>(sp + ((gz + 1 == L) ? g - LL * (L - 1) : g + LL));
-            uint32_t rnx, rny, rnz = 0u;  // nibbles: the random decision of each bond
-            if (MODEL == ISING) {
-                // Packed keying (reading 6): the 128 bits of one call serve S = 4 (2D) or 2 (3D)
-                // consecutive sites; a site's 32 / 64 bits hold one F-bit field per bond (F = 15 / 21)
-                // and, in the top bit, its cluster draw.  field < P32 >> (32 - F) decides the bond; a
-                // field equal to that value (probability 2^-F) is settled by the low bits of P32
-                // against a second call (domain TIE), so the probability is exactly P32 / 2^32.
-                constexpr int F = (DIM == 2) ? 15 : 21;
-                constexpr uint32_t FM = (1u << F) - 1u;
-                constexpr int SH2 = (DIM == 3) ? 2 * F - 32 : 0;  // field 2 inside the high word
-                const uint32_t Ptop = p.P32 >> (32 - F);
-                uint32_t f0[4], f1[4], f2[4];
-                if (DIM == 2) {
-                    const uint4 c = philox4x32_10(g >> 2, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
-                    const uint32_t cw[4] = {c.x, c.y, c.z, c.w};
-                    d = 0u;
-#pragma unroll
-                    for (int s = 0; s < 4; ++s) {
-                        f0[s] = cw[s] & FM; f1[s] = (cw[s] >> F) & FM; f2[s] = 0u;
-                        d |= (cw[s] >> 31) << s;
-                    }
-                } else {
-                    const uint4 c0 = philox4x32_10(g >> 1, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
-                    const uint4 c1 = philox4x32_10((g >> 1) + 1u, t_lo, t_hi, DOM_PACK, p.k0, p.k1);
-                    const uint32_t lo[4] = {c0.x, c0.z, c1.x, c1.z}, hi[4] = {c0.y, c0.w, c1.y, c1.w};
-                    d = 0u;
-#pragma unroll
-                    for (int s = 0; s < 4; ++s) {
-                        f0[s] = lo[s] & FM;
-                        f1[s] = __funnelshift_r(lo[s], hi[s], F) & FM;
-                        f2[s] = (hi[s] >> SH2) & FM;
-                        d |= (hi[s] >> 31) << s;
-                    }
-                }
-                // d = field - Ptop (both < 2^21): the sign bit of d is "field < Ptop", and d == 0 is a tie.
-                // Sign bits are shifted into the nibbles with one funnel shift each (sites 3..0), and the
-                // minimum of all d tells whether any field of the quad sits on the threshold.
-                rnx = rny = 0u;
-                uint32_t dmin = 0xffffffffu;
-#pragma unroll
-                for (int s = 3; s >= 0; --s) {
-                    const uint32_t d0 = f0[s] - Ptop, d1 = f1[s] - Ptop;
-                    rnx = __funnelshift_l(d0, rnx, 1);
-                    rny = __funnelshift_l(d1, rny, 1);
-                    dmin = min(dmin, min(d0, d1));
-                    if (DIM == 3) {
-                        const uint32_t d2 = f2[s] - Ptop;
-                        rnz = __funnelshift_l(d2, rnz, 1);
-                        dmin = min(dmin, d2);
-                    }
-                }
-                if (dmin == 0u) {  // probability 12 x 2^-21 per quad (3D), 8 x 2^-15 (2D)
-                    // fully unrolled: the field arrays are only ever indexed statically (registers)
-                    const uint32_t Plow = p.P32 & ((1u << (32 - F)) - 1u);
-#pragma unroll
-                    for (int s = 0; s < 4; ++s) {
-                        const bool t0 = f0[s] == Ptop, t1 = f1[s] == Ptop, t2 = DIM == 3 && f2[s] == Ptop;
-                        if (t0 || t1 || t2) {
-                            const uint4 tw = philox4x32_10(g + s, t_lo, t_hi, DOM_TIE, p.k0, p.k1);
-                            if (t0 && (tw.x >> F) < Plow) rnx |= 1u << s;
-                            if (t1 && (tw.y >> F) < Plow) rny |= 1u << s;
-                            if (t2 && (tw.z >> F) < Plow) rnz |= 1u << s;
-                        }
-                    }
-                }
-            } else {
-                const uint32_t P = p.P32;  // Potts: one call per site, word k < P32 decides bond k
-                rnx = (w[0].x < P) | ((w[1].x < P) << 1) | ((w[2].x < P) << 2) | ((w[3].x < P) << 3);
-                rny = (w[0].y < P) | ((w[1].y < P) << 1) | ((w[2].y < P) << 2) | ((w[3].y < P) << 3);
-                if (DIM == 3) rnz = (w[0].z < P) | ((w[1].z < P) << 1) | ((w[2].z < P) << 2) | ((w[3].z < P) << 3);
-                const unsigned qq = (unsigned)p.q;
-                d = 0u;
-#pragma unroll
-                for (int s = 0; s < 4; ++s) d |= (uint32_t)(((unsigned long long)w[s].w * qq) >> 32) << (s * db);
-            }
-            bxn = eq4(own, __funnelshift_r(own, nb, 8)) & rnx;
-            byn = eq4(own, up) & rny;
-            if (DIM == 3) bzn = eq4(own, fr) & rnz;
         }
-        // Ising / XY: the four 1-bit draws ride in bits 12-15 of the bond word (one register less per quad)
-        bnd[j] = bxn | (byn << 4) | (bzn << 8) | (MODEL == POTTS ? 0u : d << 12);
-        if (MODEL == POTTS) drw[j] = d;
+        // the four 1-bit draws ride in bits 12-15 of the bond word (one register less per quad)
+        bnd[j] = bxn | (byn << 4) | (bzn << 8) | (d << 12);
 
         // x-runs: link = my last site is bonded to the next quad of the row, thru = no break inside
         const uint32_t Lk = __ballot_sync(FULL, (bxn & 8u) && !rowend);
@@ -686,7 +596,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
             jump4(vlab, r, prev);
             if (k + 1 < SW_BL_JUMPS) *reinterpret_cast<uint4 *>(lab_s + li) = r;
         }
-        const uint32_t dm = (1u << db) - 1u, d = (MODEL == POTTS) ? drw[j] : (bnd[j] >> 12);
+        const uint32_t dm = (1u << db) - 1u, d = bnd[j] >> 12;
         uint4 o;
         o.x = ((tile_base + r.x) << db) | (d & dm);
         o.y = ((tile_base + r.y) << db) | ((d >> db) & dm);

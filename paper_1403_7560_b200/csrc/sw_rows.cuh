@@ -29,7 +29,7 @@
 
 namespace swk {
 
-constexpr uint32_t DOM_GROUP = 5u;   // reading 6: W_G[n] = word n % 4 of the call with counter word 3 = 5 + 256 (n / 4)
+// reading 6, domain GROUP: W_G[n] = word n % 4 of the call with counter word 3 = DOM_GROUP + 256 (n / 4)
 constexpr uint32_t GROUP_DRAW_BASE = 128u;
 
 #ifndef SW_ROW_JUMPS
@@ -58,7 +58,7 @@ struct RowGeom {
     static constexpr int OFF_DR = OFF_PM + NDIR * NROWS;    // Ising: draw mask of every row; Potts: one draw byte per site
     static constexpr int OFF_SG = OFF_DR + (MODEL == ISING ? NROWS : NS / 4);
     static constexpr int OFF_FACE = OFF_SG + (NSG + 3) / 4 * 4;
-    static constexpr int OFF_FPRE = OFF_FACE + NFWP;     // NFW prefix counts, [NFWP] = base in the pair list, [NFWP+1] = list length
+    static constexpr int OFF_FPRE = OFF_FACE + NFWP;     // NFW prefix counts, [NFWP] = base in the pair list, [NFWP+1] = list length, [NFWP+2] = its valid part
     static constexpr int OFF_LIST = OFF_FPRE + NFWP + 4; // bonds left for the union-find: (node a << 16) | node b
     static constexpr int LIST_CAP = NS / 4;
     static constexpr int WORDS = OFF_LIST + LIST_CAP;
@@ -262,7 +262,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
             if (tid == NT - 1) sg_s[TY] = sign32(reinterpret_cast<const uint4 *>(sp + x0 + grow(TY, 0)));
         }
     }
-    if (tid == 0) fpre_s[G::NFWP + 1] = 0u;
+    if (tid == 0) { fpre_s[G::NFWP + 1] = 0u; fpre_s[G::NFWP + 2] = (uint32_t)G::LIST_CAP; }
     __syncthreads();
 
     // phase 1b: bond masks of the own rows
@@ -437,7 +437,10 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                     }
                 }
             } else {
-                unfit |= 1u << r;   // list full (ordered phase with many domain walls): done after phase 2b
+                // list full (ordered phase with many domain walls): these bonds are done after phase 2b, and
+                // the list is valid only below the first reservation that did not fit
+                unfit |= 1u << r;
+                if (lane == 31) atomicMin(&fpre_s[G::NFWP + 2], base);
             }
         }
     }
@@ -448,7 +451,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
     // fetches the next bond of the warp's share, or climbs one level, or hooks -- lanes whose union needs
     // several rounds do not hold up lanes that are ready for their next bond.
     {
-        const uint32_t n = min(fpre_s[G::NFWP + 1], (uint32_t)G::LIST_CAP);
+        const uint32_t n = min(fpre_s[G::NFWP + 1], fpre_s[G::NFWP + 2]);
         uint32_t nxt = (n * (uint32_t)warp) / NW;
         const uint32_t end = (n * (uint32_t)(warp + 1)) / NW;
         const uint32_t lt = (1u << lane) - 1u;
@@ -473,7 +476,12 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                     if (old == hi) a = b;                 // done
                     else { a = old; b = lo; }             // hi was hooked meanwhile: go on from its new parent
                 } else {
-                    a = pa; b = pb;                       // climb (a == b afterwards: same tree already)
+                    // climb two levels and make both nodes skip their parents (path halving: a non-root is
+                    // never the target of a hook, and any ancestor is a valid parent)
+                    const uint32_t ga = lds_u16(lab_sa + pa), gb = lds_u16(lab_sa + pb);
+                    if (ga != pa) sts_u16(lab_sa + a, ga);
+                    if (gb != pb) sts_u16(lab_sa + b, gb);
+                    a = ga; b = gb;                       // (a == b afterwards: same tree already)
                 }
             }
         }
@@ -521,7 +529,13 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                     const int ly = wd - G::FXW - G::FYW;
                     li_j = (uint32_t)lane + 32u * (uint32_t)ly; li_i = li_j + 32u * TY * (TZ - 1); tj = tjz;
                 }
-                p.pairs[pos] = make_uint2(tile_base + li_i, (tj << G::LOG2NS) + li_j);
+                // this tile's end of the bond is handed over as the ancestor the tile-local forest gives for
+                // it (k_merge then starts its find there instead of walking the chain through L2)
+                const uint32_t ri = li_i >> 5;
+                uint32_t v = lds_u16(lab_sa + ri * 64u + 2u * run_start(bx_s[ri], (1u << (li_i & 31u)) - 1u));
+#pragma unroll
+                for (int k = 0; k < SW_ROW_JUMPS; ++k) v = lds_u16(lab_sa + v);
+                p.pairs[pos] = make_uint2(tile_base + (v >> 1), (tj << G::LOG2NS) + li_j);
             }
         }
     }
