@@ -20,13 +20,15 @@
  *   label        minimum linear site index of the site's cluster (what label equivalence with
  *                atomicMin from label = index converges to);
  *   randoms      Philox4x32-10, key = (seed low, seed high), counter = (index, t low, t high,
- *                domain), t = 0-based index of the step being executed.  Potts, XY: domain 0,
- *                index = site, word k decides bond k of the site, word 3 is the new value of the
- *                cluster rooted at the site.  Ising: domain 1, one call serves 4 (2D) or 2 (3D)
- *                consecutive sites with 15- / 21-bit fields per bond and the cluster value in the
- *                top bit of the site's piece; a field equal to the top bits of the threshold is
- *                settled by a second call (domain 4), so P(bond) is exactly floor(p 2^32) / 2^32.
- *                Domain 2: start configuration; domain 3: XY direction of step t.
+ *                domain), t = 0-based index of the step being executed (reading 6, spec
+ *                version 2).  XY, clock: domain 0, index = site, word k decides bond k of the site, the
+ *                top bit of word 3 is the draw of the cluster rooted at the site.  Ising, Potts: domain
+ *                5, index = group G = site / 32; the group's words W_G[n] = word n % 4 of the call with
+ *                counter word 3 = 5 + 256 (n / 4).  Bit b = site % 32 of W_G[1 + s dim + k] is binary digit
+ *                31 - s of the 32-bit uniform integer u(site, k); bond k is active iff the neighbours are
+ *                equal and u < floor(p 2^32).  Bit b of W_G[0]: Ising cluster draw; W_G[128 + b]: Potts
+ *                draw word (new state (w q) >> 32).  Domain 2: start configuration; domain 3: XY
+ *                direction / clock mirror of step t.
  *
  * Pointers: `sw_ctx *` is an opaque HOST pointer owned by the library.  All `host_*` arguments
  * are HOST pointers owned by the caller.  `device_workspace` (sw_create_in) is a DEVICE pointer
@@ -158,13 +160,24 @@ int sw_force_xy_phi(sw_ctx *c, int enable, double phi);
  * out[2] = unions that linked two roots, out[3] = union retries (lost atomicCAS), out[4] = total
  * find hops in the merge, out[5] = max find hops of one union, out[6] = rounds of the root-chase
  * loop in the flip kernel summed over threads (a round advances up to 4 sites by one parent), out[7] =
- * the largest such sum of one thread (16 sites). */
+ * the largest such sum of one thread (a thread owns sw_info(c, SW_INFO_FLIP_SITES_PER_THREAD) sites).
+ * Lattices that run in one CTA (SW_INFO_ONE_CTA) have no merge and no chase kernel: all zero. */
 int sw_set_counting(sw_ctx *c, int enable);
 int sw_get_label_stats(sw_ctx *c, uint64_t *host_out, int n);
 
+/* How a context runs: launch geometry chosen at create time (reported by bench.py). */
+enum { SW_INFO_TILE_X = 0, SW_INFO_TILE_Y = 1, SW_INFO_TILE_Z = 2, SW_INFO_ROWS_PER_THREAD = 3,
+       SW_INFO_FLIP_SITES_PER_THREAD = 4, SW_INFO_ONE_CTA = 5, SW_INFO_LAUNCHES_PER_STEP = 6,
+       SW_INFO_OBSERVABLES_COPY_BYTES = 7 };
+/* Returns the value, or -1 for a NULL context / unknown item.  SW_INFO_ONE_CTA = 1: lattices of at most
+ * 32768 Ising / Potts sites run all n steps of sw_step(n) in ONE launch of one CTA (sw_small.cuh);
+ * SW_INFO_LAUNCHES_PER_STEP is then 0 (one launch per call) and 3 otherwise.
+ * SW_INFO_OBSERVABLES_COPY_BYTES: device-to-host bytes of one sw_observables call. */
+long long sw_info(const sw_ctx *c, int item);
+
 /* Per-kernel device times.  With timing enabled, sw_step brackets each of the three kernels of a
- * step (k_bond_label, k_merge, k_flip) with CUDA events on the context's stream and synchronises
- * after every step (a measurement mode, slower than the asynchronous default).
+ * step (k_bond_label, k_merge, k_flip; one-CTA lattices: the whole launch in slot 0) with CUDA events on
+ * the context's stream and synchronises after every step (a measurement mode, slower than the asynchronous default).
  * sw_get_kernel_times returns the accumulated milliseconds per kernel (host_ms[0..2]) and the number
  * of steps accumulated (*host_steps) since timing was enabled, then clears the accumulators. */
 int sw_set_kernel_timing(sw_ctx *c, int enable);
@@ -174,6 +187,19 @@ int sw_get_kernel_times(sw_ctx *c, double *host_ms, int n, uint64_t *host_steps)
  * key) pairs: host_ctr = count x 4 words, host_key = count x 2 words, host_out = count x 4 words.
  * Lets the tests pin the GPU generator to the known-answer vectors. */
 int sw_philox_selftest(const uint32_t *host_ctr, const uint32_t *host_key, uint32_t *host_out, int count);
+
+/* Micro-benchmarks behind the bounds DESIGN.md section 6 quotes (test / bench only; allocate and free
+ * their own device memory, run on the legacy default stream, time `reps` launches with CUDA events after
+ * one warm-up launch and return the mean milliseconds per launch in *host_ms):
+ *   SW_MICRO_PHILOX_SITE   one Philox4x32-10 call and three threshold compares per site, one result byte
+ *                          per site written (the per-site keying of XY / clock);
+ *   SW_MICRO_PHILOX_GROUP  the transposed-digit decisions of one group of 32 sites per thread (10 calls,
+ *                          13 digits x 3 directions; the Ising / Potts keying), three mask words written;
+ *   SW_MICRO_GATHER        n dependent-free random 4-byte reads from a table of `table_words` words
+ *                          (k_merge / k_flip chase pattern), one word written per read.
+ * n = number of sites (PHILOX_*) or reads (GATHER). */
+enum { SW_MICRO_PHILOX_SITE = 0, SW_MICRO_PHILOX_GROUP = 1, SW_MICRO_GATHER = 2 };
+int sw_micro_bench(int kind, size_t n, size_t table_words, int reps, double *host_ms);
 
 #ifdef __cplusplus
 }

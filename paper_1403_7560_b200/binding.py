@@ -62,6 +62,9 @@ def lib():
     L.sw_set_kernel_timing.argtypes = [vp, i32]
     L.sw_get_kernel_times.argtypes = [vp, C.POINTER(dbl), i32, C.POINTER(u64)]
     L.sw_philox_selftest.argtypes = [vp, vp, vp, i32]
+    L.sw_info.argtypes = [vp, i32]
+    L.sw_info.restype = C.c_longlong
+    L.sw_micro_bench.argtypes = [i32, sz, sz, i32, C.POINTER(dbl)]
     _lib = L
     return _lib
 
@@ -78,6 +81,22 @@ def philox_selftest(ctr, key):
     out = np.empty_like(ctr)
     _check(lib().sw_philox_selftest(ctr.ctypes.data, key.ctypes.data, out.ctypes.data, len(ctr)))
     return out
+
+
+MICRO_PHILOX_SITE, MICRO_PHILOX_GROUP, MICRO_GATHER = 0, 1, 2
+INFO = {"tile_x": 0, "tile_y": 1, "tile_z": 2, "rows_per_thread": 3, "flip_sites_per_thread": 4, "one_cta": 5,
+        "launches_per_step": 6, "observables_copy_bytes": 7}
+
+
+def micro_bench(kind, n, table_words=0, reps=10):
+    """sw_micro_bench (include/sw.h): mean milliseconds per launch of one of the micro-benchmark kernels."""
+    ms = dbl_()
+    _check(lib().sw_micro_bench(int(kind), int(n), int(table_words), int(reps), C.byref(ms)))
+    return float(ms.value)
+
+
+def dbl_():
+    return C.c_double()
 
 
 class SwendsenWang:
@@ -107,6 +126,10 @@ class SwendsenWang:
         self.N = int(lib().sw_num_sites(self._h))
         if record_bonds:
             self.record_bonds(True)
+
+    def info(self):
+        """Launch geometry of this context (sw_info)."""
+        return {k: int(lib().sw_info(self._h, v)) for k, v in INFO.items()}
 
     def record_bonds(self, enable):
         """Steps after this call also store the bond bytes (needed by bonds())."""

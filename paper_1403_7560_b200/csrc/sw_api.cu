@@ -82,24 +82,23 @@ bool pick_ops_rows(int dim, int tx, int ty, int tz, int rows, TileOps &o)
 #ifdef SW_MENU_MIN   // developer builds: few instantiations (fast to compile)
     if (MODEL != ISING) return false;
     if (dim == 3 && ty == 32 && tz == 16) { o = make_ops_rows<3, ISING, 32, 16, 1, 8, 3>(); return true; }
-    if (dim == 2 && ty == 256) { o = make_ops_rows<2, ISING, 256, 1, 2, 4, 6>(); return true; }
+    if (dim == 2 && ty == 128) { o = make_ops_rows<2, ISING, 128, 1, 1, 4, 12>(); return true; }
     return false;
 #else
 #define SW_ROWS2(Y, RR, Q, B) if (dim == 2 && ty == Y && (rows == RR || rows == 0)) { o = make_ops_rows<2, MODEL, Y, 1, RR, Q, B>(); return true; }
 #define SW_ROWS3(Z, RR, Q, B) if (dim == 3 && ty == 32 && tz == Z && (rows == RR || rows == 0)) { o = make_ops_rows<3, MODEL, 32, Z, RR, Q, B>(); return true; }
     SW_ROWS2(32, 1, 1, 16)
+    SW_ROWS2(128, 1, 4, 12)
     SW_ROWS2(128, 2, 4, 8)
-    SW_ROWS2(128, 1, 4, 8)
+    SW_ROWS2(256, 1, 4, 6)
     SW_ROWS2(256, 2, 4, 6)
-    SW_ROWS2(256, 4, 4, 6)
-    SW_ROWS2(512, 4, 8, 3)
+    SW_ROWS2(512, 1, 8, 3)
     SW_ROWS2(512, 2, 8, 3)
-    SW_ROWS3(4, 1, 4, 8)
-    SW_ROWS3(8, 2, 4, 6)
+    SW_ROWS3(4, 1, 4, 12)
     SW_ROWS3(8, 1, 4, 6)
-    SW_ROWS3(16, 2, 8, 3)
-    SW_ROWS3(16, 4, 8, 3)
+    SW_ROWS3(8, 2, 4, 6)
     SW_ROWS3(16, 1, 8, 3)
+    SW_ROWS3(16, 2, 8, 3)
 #undef SW_ROWS2
 #undef SW_ROWS3
     return false;
@@ -157,7 +156,7 @@ void default_tile(int dim, int L, int model, int &tx, int &ty, int &tz)
     const bool rows = model == SW_ISING || model == SW_POTTS;
     if (dim == 2) {
         tz = 1;
-        if (rows) { tx = 32; ty = (L % 256 == 0) ? 256 : (L % 128 == 0 ? 128 : 32); }
+        if (rows) { tx = 32; ty = (L % 128 == 0) ? 128 : 32; }   // measured on C2 / C3: 32 x 128, one row per thread
         else if (L % 64 == 0) { tx = 64; ty = 64; }   // measured on C2 / C3 (round 1): 64x64 3 % ahead of 128x64
         else { tx = 32; ty = 32; }
     } else {
@@ -477,6 +476,10 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
         const size_t max_pairs = c->N / c->ops.tx + c->N / c->ops.ty + (dim == 3 ? c->N / c->ops.tz : 0);
         size_t blocks = (max_pairs + 255) / 256;
         if (blocks > (size_t)sms * 64) blocks = (size_t)sms * 64;
+        if (const char *env = std::getenv("SW_B200_MERGE_BLOCKS")) {   // test knob: another interleaving of the unions
+            const long v = std::atol(env);
+            if (v >= 1 && v <= 65535 * 16) blocks = (size_t)v;
+        }
         c->merge_blocks = (unsigned)blocks;
     }
     p.L = (uint32_t)L; p.N = (uint32_t)c->N;
@@ -490,6 +493,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     p.clock_T = (const uint32_t *)(base + lay.table);
     p.mirror = 0; c->mirror = 0;
     p.counting = 0;
+    p.nk_clear = (model == SW_POTTS) ? q : 0;
     c->force_phi = 0; c->forced_phi = 0.0; c->rx = c->ry = c->crefl = 0.f; c->sticky = 0;
     c->graph1 = nullptr; c->graphK = nullptr; c->graph_record = -1;
     c->series_dev = nullptr; c->series_cap = 0;
@@ -1009,6 +1013,67 @@ int sw_get_kernel_times(sw_ctx *c, double *ms, int n, uint64_t *steps)
     if (steps) *steps = c->timed_steps;
     c->timed_steps = 0;
     for (int k = 0; k < 3; ++k) c->kernel_ms[k] = 0.0;
+    return SW_OK;
+}
+
+long long sw_info(const sw_ctx *c, int item)
+{
+    if (!c) return -1;
+    switch (item) {
+    case SW_INFO_TILE_X: return c->small ? c->L : c->ops.tx;
+    case SW_INFO_TILE_Y: return c->small ? c->L : c->ops.ty;
+    case SW_INFO_TILE_Z: return c->small ? (c->dim == 3 ? c->L : 1) : c->ops.tz;
+    case SW_INFO_ROWS_PER_THREAD: return c->small ? 1 : c->ops.rows;
+    case SW_INFO_FLIP_SITES_PER_THREAD: return c->small ? 32 : (long long)c->ops.tx * c->ops.ty * c->ops.tz / c->ops.nt;
+    case SW_INFO_ONE_CTA: return c->small ? 1 : 0;
+    case SW_INFO_LAUNCHES_PER_STEP: return c->small ? 0 : 3;
+    case SW_INFO_OBSERVABLES_COPY_BYTES: return (long long)offsetof(Acc, stats);
+    default: return -1;
+    }
+}
+
+int sw_micro_bench(int kind, size_t n, size_t table_words, int reps, double *host_ms)
+{
+    if (!host_ms || reps <= 0 || n == 0 || n > 0xffffff00ull) return fail(SW_EINVAL, "sw_micro_bench: bad arguments");
+    if (kind == SW_MICRO_PHILOX_GROUP && (n % (32 * 256)) != 0) return fail(SW_EINVAL, "sw_micro_bench: n must be a multiple of 8192 sites");
+    if (kind == SW_MICRO_GATHER && (table_words == 0 || (table_words & (table_words - 1)) != 0 || table_words > 0x80000000ull))
+        return fail(SW_EINVAL, "sw_micro_bench: table_words must be a power of two");
+    void *out = nullptr, *table = nullptr;
+    const size_t out_bytes = kind == SW_MICRO_PHILOX_SITE ? n : (kind == SW_MICRO_PHILOX_GROUP ? n / 32 * 12 : n * 4);
+    cudaError_t e = cudaMalloc(&out, out_bytes);
+    if (e == cudaSuccess && kind == SW_MICRO_GATHER) {
+        e = cudaMalloc(&table, table_words * 4);
+        if (e == cudaSuccess) e = cudaMemset(table, 1, table_words * 4);
+    }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    Params p = {};
+    p.P32 = 1537996873u; p.k0 = 1u; p.k1 = 0u;   // C4's threshold
+    auto launch = [&]() {
+        if (kind == SW_MICRO_PHILOX_SITE) k_micro_philox_site<<<(unsigned)((n + 255) / 256), 256>>>((uint8_t *)out, (uint32_t)n, p.P32, p.k0, p.k1);
+        else if (kind == SW_MICRO_PHILOX_GROUP) k_micro_philox_group<<<(unsigned)(n / 32 / 256), 256>>>((uint32_t *)out, (uint32_t)(n / 32), p);
+        else k_micro_gather<<<(unsigned)((n + 255) / 256), 256>>>((const uint32_t *)table, (uint32_t)(table_words - 1), (uint32_t *)out, (uint32_t)n);
+    };
+    float ms = 0.f;
+    if (e == cudaSuccess) {
+        launch();
+        e = cudaDeviceSynchronize();
+    }
+    if (e == cudaSuccess) {
+        cudaEventRecord(e0);
+        for (int r = 0; r < reps; ++r) launch();
+        cudaEventRecord(e1);
+        e = cudaEventSynchronize(e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e == cudaSuccess) e = cudaGetLastError();
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(out);
+    cudaFree(table);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SW_ECUDA, std::string("sw_micro_bench: ") + cudaGetErrorString(e)); }
+    *host_ms = (double)ms / reps;
     return SW_OK;
 }
 

@@ -80,6 +80,7 @@ struct Params {
     const uint32_t *clock_T;      // clock: q x q bond thresholds T[u_i q + u_j] (see k_bond_label)
     int mirror;                   // clock: mirror index m of the step (the paper's ispr)
     int counting;
+    int nk_clear;                 // number of n_k accumulators k_merge clears for k_flip (Potts: q, else 0)
 };
 
 // Philox4x32-10 (Salmon et al., SC'11): 10 rounds of two 32x32->64 multiplies and a key bump.
@@ -613,10 +614,23 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
 }
 
 // ------------------------------------------------------------------------------------------------
-// Global union-find over the packed label words.  Loads bypass L1 (volatile): other CTAs update
-// parents concurrently.  A root is only ever changed by the atomicCAS that hooks it; path halving
-// rewrites non-roots with (valid) ancestors, keeping their draw field.
+// Global union-find over the packed label words.  A root is only ever changed by the atomicCAS that
+// hooks it; path splitting rewrites non-roots with (valid) ancestors, keeping their draw field.
 // ------------------------------------------------------------------------------------------------
+// Label words are read and path-split by many threads while others hook roots with atomicCAS: these
+// accesses are relaxed device-scope atomics (a word is only ever replaced by a valid word: same draw field,
+// parent = an ancestor), not plain loads and stores.
+__device__ __forceinline__ uint32_t ld_relaxed(const uint32_t *ptr)
+{
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ptr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed(uint32_t *ptr, uint32_t v)
+{
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" :: "l"(ptr), "r"(v) : "memory");
+}
+
 template <int LOG2NS, int TX, int TY>
 __device__ __forceinline__ uint32_t linear_of(const Params &p, uint32_t a)
 {
@@ -628,7 +642,7 @@ __device__ __forceinline__ uint32_t linear_of(const Params &p, uint32_t a)
 // k_merge: grid-stride loop over the compact pair list (grid: 64 CTAs per SM, i.e. one or two pairs per
 // thread, so that the list - which is in tile order - is walked in order and label blocks stay in L2).  Union of (a, b): both chains are followed in
 // one loop (two loads in flight), path splitting on the way (non-roots are re-pointed to their
-// grandparent with plain stores, keeping their draw field); then the root with the larger linear
+// grandparent with relaxed atomic stores, keeping their draw field); then the root with the larger linear
 // index is hooked under the other with atomicCAS(root word -> parent word); a lost race starts
 // over from the roots found.  Thread 0 also clears the magnetisation accumulators k_flip adds to.
 // ------------------------------------------------------------------------------------------------
@@ -637,35 +651,33 @@ __global__ void __launch_bounds__(256) k_merge(const Params p)
 {
     using G = TileGeom<DIM, TX, TY, TZ>;
     const uint32_t gid = blockIdx.x * 256u + threadIdx.x;
-    if (gid == 0) {
-        p.acc->M_int = 0ull; p.acc->mx = 0.0; p.acc->my = 0.0;
-        for (int k = 0; k < p.q; ++k) p.acc->nk[k] = 0ull;
-    }
+    if (gid == 0) { p.acc->M_int = 0ull; p.acc->mx = 0.0; p.acc->my = 0.0; }
+    if (gid < (uint32_t)p.nk_clear) p.acc->nk[gid] = 0ull;   // Potts: the accumulators k_flip adds to
     const uint32_t n = *p.npairs;
     const int db = p.db;
     const uint32_t dm = (1u << db) - 1u;
-    volatile uint32_t *vl = p.labels;
+    uint32_t *lab = p.labels;
     for (uint32_t i = gid; i < n; i += gridDim.x * 256u) {
         const uint2 ab = p.pairs[i];
         uint32_t a = ab.x, b = ab.y;
         unsigned hops = 0, retries = 0, linked = 0;
-        uint32_t wa = vl[a], wb = vl[b];
+        uint32_t wa = ld_relaxed(lab + a), wb = ld_relaxed(lab + b);
         for (;;) {
             for (;;) {
                 const uint32_t pa = wa >> db, pb = wb >> db;
                 const bool ra = pa == a, rb = pb == b;
                 if (ra && rb) break;
                 uint32_t wpa = 0u, wpb = 0u;
-                if (!ra) wpa = vl[pa];
-                if (!rb) wpb = vl[pb];
+                if (!ra) wpa = ld_relaxed(lab + pa);
+                if (!rb) wpb = ld_relaxed(lab + pb);
                 if (!ra) {
                     const uint32_t gp = wpa >> db;
-                    if (gp != pa) vl[a] = (gp << db) | (wa & dm);
+                    if (gp != pa) st_relaxed(lab + a, (gp << db) | (wa & dm));
                     a = pa; wa = wpa; ++hops;
                 }
                 if (!rb) {
                     const uint32_t gp = wpb >> db;
-                    if (gp != pb) vl[b] = (gp << db) | (wb & dm);
+                    if (gp != pb) st_relaxed(lab + b, (gp << db) | (wb & dm));
                     b = pb; wb = wpb; ++hops;
                 }
             }
@@ -731,20 +743,27 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
         const int li = (tid + j * NT) * 4;
         const uint32_t a0 = tile_base + li;
         const uint4 w4 = *reinterpret_cast<const uint4 *>(lab + a0);
-        // follow the parent words: at[s] is the node reached so far and pw[s] its word; the chase of a
-        // site ends at the node whose parent field is its own address, and that word's draw field is the
-        // cluster's new value
+        // follow the parent words to the root: the node whose parent field is its own address; that word's
+        // draw field is the cluster's new value.  First hop in straight-line code, four loads in flight: a
+        // site that is no root loads the word of its parent (the tile-local ancestor k_bond_label stored;
+        // this tile's block, usually in L1).  If that node is a root (most sites: clusters inside one
+        // tile, or whose tile-local root is the global one) the site is done; the rest goes on in a loop.
         uint32_t pw[4] = {w4.x, w4.y, w4.z, w4.w};
-        uint32_t at[4] = {a0, a0 + 1u, a0 + 2u, a0 + 3u};
+        uint32_t at[4];
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            at[s] = pw[s] >> db;
+            if (at[s] != a0 + (uint32_t)s) pw[s] = __ldg(lab + at[s]);
+        }
         for (;;) {
             const uint32_t q0 = pw[0] >> db, q1 = pw[1] >> db, q2 = pw[2] >> db, q3 = pw[3] >> db;
             const bool m0 = q0 != at[0], m1 = q1 != at[1], m2 = q2 != at[2], m3 = q3 != at[3];
+            chase_hops += counting;
             if (!(m0 | m1 | m2 | m3)) break;
             if (m0) { at[0] = q0; pw[0] = __ldg(lab + q0); }
             if (m1) { at[1] = q1; pw[1] = __ldg(lab + q1); }
             if (m2) { at[2] = q2; pw[2] = __ldg(lab + q2); }
             if (m3) { at[3] = q3; pw[3] = __ldg(lab + q3); }
-            chase_hops += counting;
         }
         __syncwarp();
 
@@ -1077,6 +1096,27 @@ __global__ void k_philox_selftest(const uint32_t *ctr, const uint32_t *key, uint
     if (i >= count) return;
     const uint4 r = philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], key[2 * i], key[2 * i + 1]);
     out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Micro-benchmarks (sw_micro_bench): the ALU cost of the random numbers alone and the rate of independent
+// random 4-byte reads, the two bounds DESIGN.md section 6 quotes next to the HBM roofline.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_micro_philox_site(uint8_t *out, uint32_t n, uint32_t P32, uint32_t k0, uint32_t k1)
+{
+    const uint32_t i = blockIdx.x * 256u + threadIdx.x;
+    if (i >= n) return;
+    const uint4 w = philox4x32_10(i, 7u, 0u, DOM_SITE, k0, k1);
+    out[i] = (uint8_t)((w.x < P32) | ((w.y < P32) << 1) | ((w.z < P32) << 2) | ((w.w >> 31) << 3));
+}
+
+__global__ void __launch_bounds__(256) k_micro_gather(const uint32_t *table, uint32_t mask, uint32_t *out, uint32_t n)
+{
+    const uint32_t i = blockIdx.x * 256u + threadIdx.x;
+    if (i >= n) return;
+    uint32_t h = i * 2654435761u;   // a cheap hash: the addresses are spread over the whole table
+    h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
+    out[i] = __ldg(table + (h & mask));
 }
 
 }  // namespace swk

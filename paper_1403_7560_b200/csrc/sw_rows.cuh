@@ -199,6 +199,15 @@ __device__ __forceinline__ void group_decisions(const Params &p, uint32_t G, uin
     }
 }
 
+// sw_micro_bench: group_decisions alone, one group of 32 sites per thread
+__global__ void __launch_bounds__(256) k_micro_philox_group(uint32_t *out, uint32_t ngroups, const Params p)
+{
+    const uint32_t G = blockIdx.x * 256u + threadIdx.x;   // ngroups is a multiple of 256 (whole warps: __any_sync)
+    uint32_t X[3], D;
+    group_decisions<3>(p, G, 7u, 0u, X, D);
+    if (G < ngroups) { out[3u * G] = X[0] ^ D; out[3u * G + 1u] = X[1]; out[3u * G + 2u] = X[2]; }
+}
+
 template <int DIM, int MODEL, int TY, int TZ, int R>
 struct RowKernelTraits {
     static constexpr int NT = (DIM == 3) ? 32 * TZ / R : TY / R;
@@ -433,7 +442,9 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                         w ^= low;
                         const uint32_t b = k.rowB + 2u * run_start(k.T, below);
                         const uint32_t a = rowP + 2u * run_start(bxP, below);
-                        list_s[pos++] = (a << 16) | b;
+                        // b has just been given a parent by this thread (a run with a further bond has a first
+                        // one): the union starts from that parent, one level up
+                        list_s[pos++] = (a << 16) | lds_u16(lab_sa + b);
                     }
                 }
             } else {
@@ -467,7 +478,10 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 }
                 nxt += __popc(need);
             }
-            if (!__any_sync(FULL, a != b)) break;
+            if (!__any_sync(FULL, a != b)) {
+                if (nxt >= end) break;
+                continue;   // every bond just fetched joins a run with its own parent: fetch again
+            }
             if (a != b) {
                 const uint32_t pa = lds_u16(lab_sa + a), pb = lds_u16(lab_sa + b);
                 if (pa == a && pb == b) {
@@ -485,6 +499,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 }
             }
         }
+    
     }
     if (fpre_s[G::NFWP + 1] > (uint32_t)G::LIST_CAP) {   // block-uniform; rare
 #pragma unroll 1

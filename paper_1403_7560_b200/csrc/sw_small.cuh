@@ -278,7 +278,10 @@ __global__ void __launch_bounds__(1024, 1) k_sw_small(const Params p, const Smal
                         }
                         nxt += __popc(need);
                     }
-                    if (!__any_sync(FULL, a != b)) break;
+                    if (!__any_sync(FULL, a != b)) {
+                        if (nxt >= end) break;
+                        continue;
+                    }
                     if (a != b) {
                         const uint32_t pa = lds_u16(lab_sa + a), pb = lds_u16(lab_sa + b);
                         if (pa == a && pb == b) {

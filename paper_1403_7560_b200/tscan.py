@@ -16,29 +16,40 @@ def moment_ratio(m2, m4):
     return float(np.mean(m4) / np.mean(m2) ** 2)
 
 
-def scan(dim, model, sizes, temperatures, n_discard=1000, n_measure=10000, seeds=(1, 2, 3, 4), q=0):
+def _one_chain(dim, L, model, q, T, seed, n_discard, n_measure):
+    """One (L, T, seed) chain on a context with its own CUDA stream (library-owned memory and stream)."""
+    g = binding.SwendsenWang(dim, L, model, q, 1.0 / T, seed=seed, use_torch=False)
+    g.step(n_discard)
+    s = g.run_series(n_measure)
+    g.close()
+    N = L ** dim
+    return moment_ratio(s["M2"], s["M4"]), float(np.mean(s["E"])) / N, float(np.mean(s["M2"])) / N ** 2
+
+
+def scan(dim, model, sizes, temperatures, n_discard=1000, n_measure=10000, seeds=(1, 2, 3, 4), q=0, concurrent=16):
     """U(L, T), E/N and <M^2>/N^2 with errors from the spread over independent seeds.
 
+    The paper's workflow is many temperatures x four independent runs: all (T, seed) chains
+    of a size are independent, so up to `concurrent` of them are live at once, each on its own context and CUDA
+    stream, driven by host threads (the C calls release the GIL).  Small lattices, which run in one CTA
+    (sw_small.cuh) or are launch-bound, then share the GPU instead of queueing behind each other; the result
+    does not depend on `concurrent` (same seeds, same series).
+
     Returns {L: {"T": array, "U": array, "U_err": array, "E": array, "E_err": array, "M2": array}}."""
+    from concurrent.futures import ThreadPoolExecutor
     out = {}
-    for L in sizes:
-        N = L ** dim
-        rows = []
-        for T in temperatures:
-            us, es, m2s = [], [], []
-            for seed in seeds:
-                g = binding.SwendsenWang(dim, L, model, q, 1.0 / T, seed=seed)
-                g.step(n_discard)
-                s = g.run_series(n_measure)
-                g.close()
-                us.append(moment_ratio(s["M2"], s["M4"]))
-                es.append(float(np.mean(s["E"])) / N)
-                m2s.append(float(np.mean(s["M2"])) / N ** 2)
-            k = len(seeds)
-            rows.append((T, np.mean(us), np.std(us, ddof=1) / np.sqrt(k) if k > 1 else 0.0,
-                         np.mean(es), np.std(es, ddof=1) / np.sqrt(k) if k > 1 else 0.0, np.mean(m2s)))
-        a = np.array(rows, dtype=np.float64)
-        out[L] = {"T": a[:, 0], "U": a[:, 1], "U_err": a[:, 2], "E": a[:, 3], "E_err": a[:, 4], "M2": a[:, 5]}
+    with ThreadPoolExecutor(max_workers=max(1, int(concurrent))) as pool:
+        for L in sizes:
+            jobs = {(T, seed): pool.submit(_one_chain, dim, L, model, q, T, seed, n_discard, n_measure)
+                    for T in temperatures for seed in seeds}
+            rows = []
+            for T in temperatures:
+                us, es, m2s = zip(*[jobs[(T, seed)].result() for seed in seeds])
+                k = len(seeds)
+                rows.append((T, np.mean(us), np.std(us, ddof=1) / np.sqrt(k) if k > 1 else 0.0,
+                             np.mean(es), np.std(es, ddof=1) / np.sqrt(k) if k > 1 else 0.0, np.mean(m2s)))
+            a = np.array(rows, dtype=np.float64)
+            out[L] = {"T": a[:, 0], "U": a[:, 1], "U_err": a[:, 2], "E": a[:, 3], "E_err": a[:, 4], "M2": a[:, 5]}
     return out
 
 

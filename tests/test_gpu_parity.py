@@ -83,11 +83,50 @@ def test_full_trajectory_bit_exact(dim, L, model, q, T, steps):
     assert (e, m, m2, m4) == pytest.approx(o.observables(), rel=1e-14)
 
 
+@pytest.mark.parametrize("dim,L,model,q,T,steps", [(2, 32, 0, 0, TC2, 100), (2, 64, 0, 0, TC2, 200), (2, 96, 0, 0, TC2, 40), (3, 32, 0, 0, T3, 40),
+                                                     (2, 128, 1, 3, TP3, 40), (3, 32, 1, 5, 1.4, 20), (2, 160, 1, 2, 1.1, 20)])
+def test_small_lattices_on_the_tile_path(dim, L, model, q, T, steps, monkeypatch):
+    """Lattices of at most 32768 Ising / Potts sites normally take the one-CTA kernel (sw_small.cuh); with
+    SW_B200_NO_SMALL they run the three-kernel tile path, where a lattice of one or a few tiles sends every
+    periodic-wrap bond through the global merge (a tile that is its own neighbour)."""
+    sw, orc = _mods()
+    monkeypatch.setenv("SW_B200_NO_SMALL", "1")
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=1, record_bonds=True)
+    o = orc.Oracle(dim, L, model, q, 1.0 / T, 1)
+    for t in range(steps):
+        g.step(1)
+        o.step(1)
+        _compare_step(g, o, f"tile path dim{dim} L{L} model{model} t={t}")
+    g.step(7)
+    o.step(7)
+    assert np.array_equal(g.spins(), o.spins()) and g.counts() == o.counts()
+    sg, so_ = g.run_series(9), o.run_series(9)
+    assert np.array_equal(sg["E"], so_["E"]) and np.array_equal(sg["M2"], so_["M2"])
+
+
+def test_one_cta_kernel_many_steps_per_launch():
+    """sw_small.cuh: sw_step(n) and sw_run_series(n) are ONE launch for n steps; against n oracle steps, and
+    cluster statistics / labels of the last step."""
+    sw, orc = _mods()
+    for dim, L, model, q, T in [(2, 64, 0, 0, TC2), (2, 160, 0, 0, TC2), (3, 32, 0, 0, T3), (2, 96, 1, 4, 0.9), (3, 32, 1, 3, 1.8)]:
+        g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=6, record_bonds=True)
+        o = orc.Oracle(dim, L, model, q, 1.0 / T, 6)
+        g.step(37)
+        o.step(37)
+        _compare_step(g, o, f"one-CTA kernel dim{dim} L{L} model{model}, 37 steps in one launch")
+        sg, so_ = g.run_series(25), o.run_series(25)
+        assert np.array_equal(sg["E"], so_["E"]) and np.array_equal(sg["M"], so_["M"]) and np.array_equal(sg["M2"], so_["M2"])
+        _compare_step(g, o, "after the series")
+        ncl, s2 = g.cluster_stats()
+        assert ncl == int(so_["n_clusters"][-1]) and s2 == int(so_["sum_nc2"][-1])
+        g.close()
+
+
 # Tile menus.  Ising / Potts run the row kernel (tiles 32 x TY (x TZ), R rows per thread: SW_B200_TILE,
 # SW_B200_ROWS), XY / clock the quad kernel; small lattices would silently take the smallest tile, so every
 # instantiation bench.py can time is forced here by name.
-ROW_TILES_2D = [("32x32", 1), ("32x128", 1), ("32x128", 2), ("32x256", 2), ("32x256", 4), ("32x512", 2), ("32x512", 4)]
-ROW_TILES_3D = [("32x32x4", 1), ("32x32x8", 1), ("32x32x8", 2), ("32x32x16", 1), ("32x32x16", 2), ("32x32x16", 4)]
+ROW_TILES_2D = [("32x32", 1), ("32x128", 1), ("32x128", 2), ("32x256", 1), ("32x256", 2), ("32x512", 1), ("32x512", 2)]
+ROW_TILES_3D = [("32x32x4", 1), ("32x32x8", 1), ("32x32x8", 2), ("32x32x16", 1), ("32x32x16", 2)]
 
 
 @pytest.mark.parametrize("model,q,T", [(0, 0, TC2), (1, 3, TP3), (1, 9, 0.8)])
@@ -320,27 +359,52 @@ def test_xy_statistics_against_oracle_3sigma():
 # recording off); the oracle needs 2-20 s per step there, so single steps are compared by state
 # injection: a step is a deterministic function of (spins, t).
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("name,gpu_steps", [("C2", 60), ("C3", 60), ("C4", 40), ("C5", 30)])
-def test_full_size_config_sampled_step(name, gpu_steps):
+def _compare_injected(g, o, model, dim, L, tag):
+    """One step on both sides from the same state (the oracle takes the GPU's spins and step index), in the
+    launch configuration bench.py times (bond recording off).  Ising / Potts / clock: labels, spins and the
+    integer sums must be identical.  XY: identical wherever no bond decision straddles fp32 / fp64."""
+    o.set_spins(g.spins(), g.t)
+    g.step(1)
+    o.step(1)
+    if model == 2:
+        if np.array_equal(g.labels(), o.labels()):
+            assert np.array_equal(g.spins(), o.spins()), f"{tag}: angles differ although the clusters agree"
+            return 0
+        return 1
+    assert np.array_equal(g.labels(), o.labels()), f"{tag}: labels differ"
+    assert np.array_equal(g.spins(), o.spins()), f"{tag}: spins differ"
+    if model == 3:
+        Dg, ng = g.clock_hist()
+        Do, no = o.clock_hist()
+        assert g.clock_mirror() == o.clock_mirror() and np.array_equal(Dg, Do) and np.array_equal(ng, no), f"{tag}: clock histograms differ"
+    else:
+        assert g.counts() == o.counts(), f"{tag}: integer E / M differ"
+    return 0
+
+
+@pytest.mark.parametrize("name,burn", [("C2", 80), ("C3", 80), ("C4", 60), ("C5", 40), ("X1", 40), ("X2", 60), ("X3", 40)])
+def test_full_size_config_sampled_steps(name, burn):
+    """SURVEY.md 8(c) protocol at full size: steps 0-2 from the seeded start, then three consecutive steps from
+    the (nearly) thermalised state reached after `burn` GPU steps, each compared by state injection."""
     sw, orc = _mods()
     from paper_1403_7560_b200 import inputs
-    cfg = inputs.CONFIGS[name]
+    cfg = {**inputs.CONFIGS, **inputs.EXTRA_CONFIGS}[name]
     dim, L, model, q, T = cfg["dim"], cfg["L"], cfg["model"], cfg["q"], cfg["T"]
     g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=1)
     o = orc.Oracle(dim, L, model, q, 1.0 / T, 1)
     first = g.spins()
     assert np.array_equal(first, o.spins()), "seeded start differs"
     del first
-    g.step(gpu_steps)                      # towards the critical state: large tile-crossing clusters
-    o.set_spins(g.spins(), g.t)
-    g.step(1)
-    o.step(1)
+    straddles = 0
+    for t in range(3):
+        straddles += _compare_injected(g, o, model, dim, L, f"{name} t={t}")
+    g.step(burn)                           # towards the critical state: large tile-crossing clusters
+    for t in range(3):
+        straddles += _compare_injected(g, o, model, dim, L, f"{name} t={burn + 3 + t}")
     if model == 2:
-        # XY: the step just taken ran without bond recording (bench configuration); a second injected
-        # step with recording on gives the bond mismatch count
-        same = np.array_equal(g.labels(), o.labels())
-        if same:
-            assert np.array_equal(g.spins(), o.spins())
+        # XY: a step whose clusters differ must be explained by bond decisions that straddle fp32 / fp64: count
+        # them on one more injected step with recording on (north_star: <= 1e-6 of the bonds)
+        assert straddles <= 3
         g.record_bonds(True)
         o.set_spins(g.spins(), g.t)
         g.step(1)
@@ -349,11 +413,89 @@ def test_full_size_config_sampled_step(name, gpu_steps):
         assert bad <= max(1, int(1e-6 * dim * L ** dim)), f"{bad} mismatching bond bytes"
         if bad == 0:
             assert np.array_equal(g.labels(), o.labels()) and np.array_equal(g.spins(), o.spins())
-    else:
-        assert np.array_equal(g.labels(), o.labels()), "labels differ"
-        assert np.array_equal(g.spins(), o.spins()), "spins differ"
-        assert g.counts() == o.counts(), "integer E / M differ"
     g.close()
+
+
+@pytest.mark.parametrize("dim,L,model,q,Tc", [(2, 4096, 0, 0, TC2), (3, 256, 0, 0, T3), (2, 4096, 1, 3, TP3)])
+def test_ordered_phase_at_scale(dim, L, model, q, Tc):
+    """The other extreme of the labelling cost (SURVEY.md 8(d) stress inputs; PAPER.md:176-195 scans below T_c):
+    a cold start at beta = 40 (every bond active: one cluster, label 0 everywhere, every tile-face bond goes
+    through the global merge and contends for one root) and the state reached at T = 0.8 T_c (one giant
+    cluster plus a gas of small ones), both against the oracle."""
+    sw, orc = _mods()
+    from paper_1403_7560_b200 import inputs
+    N = L ** dim
+    g = sw.SwendsenWang(dim, L, model, q, 40.0, seed=3)
+    o = orc.Oracle(dim, L, model, q, 40.0, 3)
+    cold = inputs.aligned_spins(model, N)
+    g.set_spins(cold, 5)
+    g.step(1)
+    lab = g.labels()
+    assert not lab.any(), "cold start at beta = 40: one cluster with label 0"
+    assert len(np.unique(g.spins())) == 1
+    del lab
+    g.set_spins(cold, 5)
+    _compare_injected(g, o, model, dim, L, "cold start")
+    g.close()
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / (0.8 * Tc), seed=4)
+    o = orc.Oracle(dim, L, model, q, 1.0 / (0.8 * Tc), 4)
+    g.set_spins(cold, 0)
+    g.step(30)
+    for t in range(2):
+        _compare_injected(g, o, model, dim, L, f"T = 0.8 Tc t={t}")
+    g.close()
+
+
+def test_cold_start_3d_512():
+    """Cold start at C4's size: 2^27 sites in one cluster, 25 million tile-face unions onto one root."""
+    sw, _ = _mods()
+    from paper_1403_7560_b200 import inputs
+    g = sw.SwendsenWang(3, 512, 0, 0, 40.0, seed=3)
+    g.set_spins(inputs.aligned_spins(0, 512 ** 3), 5)
+    g.step(1)
+    assert not g.labels().any()
+    s = g.spins()
+    assert (s == s[0]).all()
+    e, m = g.counts()
+    assert e == -3 * 512 ** 3 and abs(m[0]) == 512 ** 3
+    g.close()
+
+
+def test_potts_largest_q_at_full_size():
+    """Boundary case of the label word: 2D L = 4096 with q = 255 -- 2^24 addresses x 2^8 draw bits fill the
+    32 bits exactly (include/sw.h)."""
+    sw, orc = _mods()
+    g = sw.SwendsenWang(2, 4096, 1, 255, 1.0 / 0.45, seed=2)
+    o = orc.Oracle(2, 4096, 1, 255, 1.0 / 0.45, 2)
+    assert np.array_equal(g.spins(), o.spins())
+    for t in range(3):
+        _compare_injected(g, o, 1, 2, 4096, f"q=255 t={t}")
+    g.close()
+
+
+def test_gpu_energy_against_kaufman_at_config_2_size():
+    """SURVEY.md 8(c) pin P5 at the size of BASELINE config 2: 2D Ising L = 4096 at T = 2.269185, four seeds
+     x 2 10^4 measured steps after 2000 discarded: <E>/N against Kaufman's exact finite-torus
+    value -1.41436686099655 within 3 sigma, and resolved from Onsager's L -> infinity value -sqrt 2."""
+    import os
+    sw, _ = _mods()
+    from stats import binned_mean_err, golden_rows
+    rows = golden_rows(os.path.join(os.path.dirname(__file__), "golden", "kaufman_energy.txt"))
+    e_exact = [float(r[2]) for r in rows if int(r[0]) == 4096][0]
+    N = 4096 * 4096
+    means, errs = [], []
+    for seed in (1, 2, 3, 4):
+        g = sw.SwendsenWang(2, 4096, 0, 0, 1.0 / TC2, seed=seed)
+        g.step(2000)
+        s = g.run_series(20000)
+        m, e = binned_mean_err(s["E"] / N, 50)
+        means.append(m)
+        errs.append(e)
+        g.close()
+    mean = float(np.mean(means))
+    err = float(np.sqrt(np.sum(np.square(errs))) / len(errs))
+    assert abs(mean - e_exact) <= 3.0 * err, f"E/N = {mean} +- {err}, exact {e_exact}"
+    assert abs(mean + math.sqrt(2.0)) > 3.0 * err, f"E/N = {mean} +- {err} not resolved from -sqrt(2)"
 
 
 def test_recording_does_not_change_the_trajectory():
@@ -436,8 +578,18 @@ def test_temperature_scan_moment_ratio_crossing():
     L = 64 crosses near T_c = 4.51151 at U* ~ 1.6; U falls towards 1 below and rises
     towards 3 above T_c, faster for the larger lattice.  Wide tolerances: corrections to scaling at
     these sizes shift the crossing by ~0.01 in T."""
+    import time
     from paper_1403_7560_b200 import tscan
     Ts = [4.40, 4.47, 4.50, 4.52, 4.55, 4.62]
+    # chains on separate streams (SURVEY.md 8(f)4 "replicas across streams") give the same numbers as one
+    # chain after the other: same seeds, same series; the wall times of both are printed for the report
+    t0 = time.perf_counter()
+    r1 = tscan.scan(3, 0, [32], Ts[:2], n_discard=300, n_measure=2000, concurrent=1)
+    t1 = time.perf_counter()
+    r8 = tscan.scan(3, 0, [32], Ts[:2], n_discard=300, n_measure=2000, concurrent=8)
+    t2 = time.perf_counter()
+    assert np.array_equal(r1[32]["U"], r8[32]["U"]) and np.array_equal(r1[32]["E"], r8[32]["E"])
+    print(f"tscan 8 chains of 3D L=32, 2300 steps each: serial {t1 - t0:.2f} s, 8 streams {t2 - t1:.2f} s")
     r = tscan.scan(3, 0, [32, 64], Ts, n_discard=1500, n_measure=15000)
     for L in (32, 64):
         assert np.all(np.diff(r[L]["U"]) > 0), "U(T) must increase with T across the transition"
@@ -586,7 +738,8 @@ def test_contexts_are_independent():
     assert a.counts() == ref_a.counts() and b.counts() == ref_b.counts()
 
 
-@pytest.mark.parametrize("dim,L,model,q,T", [(3, 128, 0, 0, T3), (2, 1024, 0, 0, TC2), (3, 96, 3, 64, 2.2)])
+@pytest.mark.parametrize("dim,L,model,q,T", [(3, 128, 0, 0, T3), (2, 1024, 0, 0, TC2), (3, 96, 3, 64, 2.2), (2, 4096, 0, 0, TC2),
+                                            (3, 512, 0, 0, T3), (2, 4096, 1, 3, TP3), (3, 256, 2, 0, 2.2019)])
 def test_repeated_step_is_deterministic(dim, L, model, q, T):
     """The lock-free union-finds run in a different order every time; the result must not depend on it:
     the same step from the same state, 12 times, gives identical labels and spins (I6)."""
@@ -603,3 +756,31 @@ def test_repeated_step_is_deterministic(dim, L, model, q, T):
             ref_labels, ref_spins = labels, spins
         else:
             assert np.array_equal(labels, ref_labels) and np.array_equal(spins, ref_spins), f"repeat {k} differs"
+
+
+@pytest.mark.parametrize("blocks", [1, 7, 148, 4096])
+@pytest.mark.parametrize("dim,L,model,q,T", [(2, 512, 0, 0, 1.9), (3, 96, 0, 0, 3.9), (2, 512, 1, 3, 0.9)])
+def test_merge_is_order_independent_stress(dim, L, model, q, T, blocks, monkeypatch):
+    """The global union-find path-splits label words with relaxed atomic stores while other threads hook
+    roots with atomicCAS: giant-cluster, striped and domain states, each stepped 6 times from
+    the same state with a different k_merge grid (SW_B200_MERGE_BLOCKS: from one CTA walking the whole pair
+    list to one pair per thread), must give the oracle's labels every time."""
+    sw, orc = _mods()
+    from paper_1403_7560_b200 import inputs
+    monkeypatch.setenv("SW_B200_MERGE_BLOCKS", str(blocks))
+    monkeypatch.setenv("SW_B200_NO_SMALL", "1")
+    N = L ** dim
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=17)
+    o = orc.Oracle(dim, L, model, q, 1.0 / T, 17)
+    states = [inputs.aligned_spins(model, N), inputs.striped_spins(model, dim, L, 7, max(q, 2)),
+              inputs.domain_spins(model, dim, L, 40, max(q, 2), seed=3)]
+    for k, st in enumerate(states):
+        o.set_spins(st, 10 * k)
+        o.step(1)
+        want_labels, want_spins = o.labels(), o.spins()
+        for rep in range(6):
+            g.set_spins(st, 10 * k)
+            g.step(1)
+            assert np.array_equal(g.labels(), want_labels), f"state {k} repeat {rep}: labels differ"
+            assert np.array_equal(g.spins(), want_spins), f"state {k} repeat {rep}: spins differ"
+    g.close()
