@@ -80,8 +80,11 @@ bool pick_ops_rows(int dim, int tx, int ty, int tz, int rows, TileOps &o)
 {
     if (tx != 32) return false;
 #ifdef SW_MENU_MIN   // developer builds: few instantiations (fast to compile)
+#ifndef SW_EXP_FLIP_QPT
+#define SW_EXP_FLIP_QPT 8
+#endif
     if (MODEL != ISING) return false;
-    if (dim == 3 && ty == 32 && tz == 16) { o = make_ops_rows<3, ISING, 32, 16, 1, 8, 3>(); return true; }
+    if (dim == 3 && ty == 32 && tz == 16) { o = make_ops_rows<3, ISING, 32, 16, 1, SW_EXP_FLIP_QPT, 3>(); return true; }
     if (dim == 2 && ty == 128) { o = make_ops_rows<2, ISING, 128, 1, 1, 4, 12>(); return true; }
     return false;
 #else
@@ -105,7 +108,25 @@ bool pick_ops_rows(int dim, int tx, int ty, int tz, int rows, TileOps &o)
 #endif
 }
 
-// Tile menu of the quad kernel (XY, clock).  Tile sides are powers of two, TX in {32, 64, 128}; every side
+// XY, clock on the row kernel: one row per thread only (the warp makes the masks of its 32 rows together).
+template <int MODEL>
+bool pick_ops_rows1(int dim, int tx, int ty, int tz, TileOps &o)
+{
+    if (tx != 32) return false;
+#ifdef SW_MENU_MIN
+    return false;
+#else
+    if (dim == 2 && ty == 32) { o = make_ops_rows<2, MODEL, 32, 1, 1, 1, 16>(); return true; }
+    if (dim == 2 && ty == 128) { o = make_ops_rows<2, MODEL, 128, 1, 1, 4, 12>(); return true; }
+    if (dim == 2 && ty == 256) { o = make_ops_rows<2, MODEL, 256, 1, 1, 4, 6>(); return true; }
+    if (dim == 3 && ty == 32 && tz == 4) { o = make_ops_rows<3, MODEL, 32, 4, 1, 4, 12>(); return true; }
+    if (dim == 3 && ty == 32 && tz == 8) { o = make_ops_rows<3, MODEL, 32, 8, 1, 4, 6>(); return true; }
+    if (dim == 3 && ty == 32 && tz == 16) { o = make_ops_rows<3, MODEL, 32, 16, 1, 8, 3>(); return true; }
+    return false;
+#endif
+}
+
+// Tile menu of the quad kernel (XY, clock; round-1 kernel, kept selectable with SW_B200_KERNEL=quad).  Tile sides are powers of two, TX in {32, 64, 128}; every side
 // must divide L.
 template <int MODEL>
 bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
@@ -128,6 +149,19 @@ bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
     return false;
 }
 
+// Which bond / label kernel a model runs: Ising and Potts always the row kernel (sw_rows.cuh); the clock
+// model the row kernel by default, XY the quad kernel by default (measured: the row kernel has to compute
+// the projection of the +z neighbour a second time, which costs XY more than the cheaper labelling saves:
+// C5 0.341 vs 0.286 ms per step; clock X3 0.249 vs 0.260).  SW_B200_KERNEL=rows|quad forces one of them.
+bool use_rows(int model)
+{
+    if (model == SW_ISING || model == SW_POTTS) return true;
+    const char *kern = std::getenv("SW_B200_KERNEL");
+    if (kern && std::strcmp(kern, "quad") == 0) return false;
+    if (kern && std::strcmp(kern, "rows") == 0) return true;
+    return model == SW_CLOCK;
+}
+
 // Small lattices (fewer tiles than the GPU has room for): what counts is the critical path of one CTA,
 // so the smallest tile of the menu with the fewest sites per thread.
 bool pick_ops_small_model(int model, int dim, TileOps &o)
@@ -137,23 +171,28 @@ bool pick_ops_small_model(int model, int dim, TileOps &o)
 #endif
     if (model == SW_ISING) return pick_ops_rows<ISING>(dim, 32, 32, dim == 3 ? 4 : 1, 1, o);
     if (model == SW_POTTS) return pick_ops_rows<POTTS>(dim, 32, 32, dim == 3 ? 4 : 1, 1, o);
-    if (model == SW_CLOCK) { if (dim == 2) o = make_ops<2, CLOCK, 32, 32, 1, 1>(); else o = make_ops<3, CLOCK, 32, 8, 8, 1>(); return true; }
-    if (dim == 2) o = make_ops<2, XY, 32, 32, 1, 1>(); else o = make_ops<3, XY, 32, 8, 8, 1>();
-    return true;
+    if (!use_rows(model)) {
+        if (model == SW_CLOCK) { if (dim == 2) o = make_ops<2, CLOCK, 32, 32, 1, 1>(); else o = make_ops<3, CLOCK, 32, 8, 8, 1>(); return true; }
+        if (dim == 2) o = make_ops<2, XY, 32, 32, 1, 1>(); else o = make_ops<3, XY, 32, 8, 8, 1>();
+        return true;
+    }
+    if (model == SW_CLOCK) return pick_ops_rows1<CLOCK>(dim, 32, 32, dim == 3 ? 4 : 1, o);
+    return pick_ops_rows1<XY>(dim, 32, 32, dim == 3 ? 4 : 1, o);
 }
 
 bool pick_ops_model(int model, int dim, int tx, int ty, int tz, int rows, TileOps &o)
 {
     if (model == SW_ISING) return pick_ops_rows<ISING>(dim, tx, ty, tz, rows, o);
     if (model == SW_POTTS) return pick_ops_rows<POTTS>(dim, tx, ty, tz, rows, o);
-    if (model == SW_CLOCK) return pick_ops<CLOCK>(dim, tx, ty, tz, o);
-    return pick_ops<XY>(dim, tx, ty, tz, o);
+    const bool quad = !use_rows(model);
+    if (model == SW_CLOCK) return quad ? pick_ops<CLOCK>(dim, tx, ty, tz, o) : pick_ops_rows1<CLOCK>(dim, tx, ty, tz, o);
+    return quad ? pick_ops<XY>(dim, tx, ty, tz, o) : pick_ops_rows1<XY>(dim, tx, ty, tz, o);
 }
 
 // Default tile of a lattice (SW_B200_TILE=TXxTYxTZ and SW_B200_ROWS=R override it: tuning knobs).
 void default_tile(int dim, int L, int model, int &tx, int &ty, int &tz)
 {
-    const bool rows = model == SW_ISING || model == SW_POTTS;
+    const bool rows = use_rows(model);
     if (dim == 2) {
         tz = 1;
         if (rows) { tx = 32; ty = (L % 128 == 0) ? 128 : 32; }   // measured on C2 / C3: 32 x 128, one row per thread

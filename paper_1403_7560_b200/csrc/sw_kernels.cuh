@@ -702,14 +702,27 @@ __global__ void __launch_bounds__(256) k_merge(const Params p)
     }
 }
 
+__device__ __forceinline__ uint4 ldg_stream(const uint32_t *ptr)
+{
+    uint4 v;
+    asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(ptr) : "memory");
+    return v;
+}
+
 // ------------------------------------------------------------------------------------------------
 // k_flip: one CTA per tile, QPT quads per thread.  Every site follows its parent words to the root
 // (first hop: the tile-local root, whose word sits in this tile's 4*NS-byte block and is served by
 // L1; further hops only for clusters that cross tile faces), takes the root's draw field as the
 // cluster's new value and writes its spin; magnetisation sums per CTA.
 // ------------------------------------------------------------------------------------------------
+#ifndef SW_FLIP_PREFETCH
+#define SW_FLIP_PREFETCH 1   // quads whose label words are in flight ahead of the chase
+#endif
+#ifndef SW_FLIP_THREADS_PER_SM
+#define SW_FLIP_THREADS_PER_SM 2048  // resident threads per SM k_flip is compiled for (register cap)
+#endif
 template <int DIM, int MODEL, int TX, int TY, int TZ, int NT>
-__global__ void __launch_bounds__(NT) k_flip(const Params p)
+__global__ void __launch_bounds__(NT, (SW_FLIP_THREADS_PER_SM / NT > 0 ? SW_FLIP_THREADS_PER_SM / NT : 1)) k_flip(const Params p)
 {
     using G = TileGeom<DIM, TX, TY, TZ>;
     constexpr int NS = G::NS, NQ = NS / 4, QPT = NQ / NT;
@@ -738,11 +751,25 @@ __global__ void __launch_bounds__(NT) k_flip(const Params p)
     int m_loc = 0;
     uint32_t cnt_lo = 0u, cnt_hi = 0u;  // Potts, q <= 8: per-thread counts of states 0-3 / 4-7, one byte each
     unsigned chase_hops = 0;
+    // the label words of the NEXT quad are requested before the parents of this one are followed: the
+    // kernel is bound by the latency of these reads (DRAM), not by instruction issue
+#if SW_FLIP_PREFETCH == 2
+    uint4 w4n = ldg_stream(lab + tile_base + tid * 4), w4m = w4n;
+    if (QPT > 1) w4m = ldg_stream(lab + tile_base + (tid + NT) * 4);
+#else
+    uint4 w4n = ldg_stream(lab + tile_base + tid * 4);
+#endif
 #pragma unroll
     for (int j = 0; j < QPT; ++j) {
         const int li = (tid + j * NT) * 4;
         const uint32_t a0 = tile_base + li;
-        const uint4 w4 = *reinterpret_cast<const uint4 *>(lab + a0);
+        const uint4 w4 = w4n;
+#if SW_FLIP_PREFETCH == 2
+        w4n = w4m;
+        if (j + 2 < QPT) w4m = ldg_stream(lab + a0 + 2 * NT * 4);
+#else
+        if (j + 1 < QPT) w4n = ldg_stream(lab + a0 + NT * 4);
+#endif
         // follow the parent words to the root: the node whose parent field is its own address; that word's
         // draw field is the cluster's new value.  First hop in straight-line code, four loads in flight: a
         // site that is no root loads the word of its parent (the tile-local ancestor k_bond_label stored;

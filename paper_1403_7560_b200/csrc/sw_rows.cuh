@@ -56,7 +56,7 @@ struct RowGeom {
     static constexpr int OFF_BX = NS / 2;                   // after the 16-bit parent entries: Bx of every row (face bit cleared)
     static constexpr int OFF_PM = OFF_BX + NROWS;           // pending masks [dir][row]
     static constexpr int OFF_DR = OFF_PM + NDIR * NROWS;    // Ising: draw mask of every row; Potts: one draw byte per site
-    static constexpr int OFF_SG = OFF_DR + (MODEL == ISING ? NROWS : NS / 4);
+    static constexpr int OFF_SG = OFF_DR + (MODEL != POTTS ? NROWS : NS / 4);
     static constexpr int OFF_FACE = OFF_SG + (NSG + 3) / 4 * 4;
     static constexpr int OFF_FPRE = OFF_FACE + NFWP;     // NFW prefix counts, [NFWP] = base in the pair list, [NFWP+1] = list length, [NFWP+2] = its valid part
     static constexpr int OFF_LIST = OFF_FPRE + NFWP + 4; // bonds left for the union-find: (node a << 16) | node b
@@ -103,6 +103,12 @@ __device__ __forceinline__ uint32_t lds_u16(uint32_t saddr)
     uint16_t v;
     asm volatile("ld.volatile.shared.u16 %0, [%1];" : "=h"(v) : "r"(saddr) : "memory");
     return (uint32_t)v;
+}
+// v <- 16-bit shared[saddr] if flag != 0 (predicated: no branch, no shared-memory wavefront when off)
+__device__ __forceinline__ void lds_u16_if(uint32_t &v, uint32_t flag, uint32_t saddr)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %1, 0;\n\t@p ld.shared.u16 %0, [%2];\n\t}"
+                 : "+r"(v) : "r"(flag), "r"(saddr) : "memory");
 }
 __device__ __forceinline__ void sts_u16(uint32_t saddr, uint32_t v)
 {
@@ -171,9 +177,10 @@ __device__ __forceinline__ void group_decisions(const Params &p, uint32_t G, uin
             const int n = 4 * c + j;
             if (n == 0) { D = w[0]; continue; }
             const int s = (n - 1) / DIM, k = (n - 1) % DIM;
-            const uint32_t pm = (uint32_t)((int32_t)(P << s) >> 31);   // digit 31 - s of P32, spread over the word
-            X[k] |= U[k] & ~w[j] & pm;                                  // digit of u is 0, digit of P32 is 1: u < P32
-            U[k] &= ~(w[j] ^ pm);                                       // digits equal: still undecided
+            // digit 31 - s of P32 (warp-uniform): 1 -> sites whose digit is 0 are decided "u < P32", the others
+            // stay undecided; 0 -> sites whose digit is 1 are decided "u > P32", the others stay undecided
+            if ((P >> (31 - s)) & 1u) { X[k] |= U[k] & ~w[j]; U[k] &= w[j]; }
+            else U[k] &= ~w[j];
         }
     }
     uint32_t und = U[0] | U[1] | (DIM == 3 ? U[2] : 0u);
@@ -221,7 +228,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
     using G = RowGeom<DIM, MODEL, TY, TZ>;
     constexpr int NT = RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT;
     constexpr int NROWS = G::NROWS, NW = NT / 32;
-    static_assert(MODEL == ISING || MODEL == POTTS, "constant bond probability");
+    static_assert(R == 1 || MODEL == ISING || MODEL == POTTS, "XY / clock: the 32 threads of a warp make the masks of their 32 rows together");
     extern __shared__ __align__(16) uint32_t smem_u32[];
     uint32_t *lab_s = smem_u32;                       // 16-bit parent entries, one per site: node of the parent
     uint32_t *bx_s = smem_u32 + G::OFF_BX;
@@ -280,6 +287,68 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
         const int ly = row_y(r), lz = row_z(r);
         const int row = ly + TY * lz;
         const uint32_t g0 = grow(ly, lz);
+        uint32_t Bx, By, Bz = 0u, D = 0u;
+        if (MODEL == XY || MODEL == CLOCK) {
+            // XY (Wolff embedding) and the q-state clock model (readings 23-25): the bond
+            // probability depends on the two spins, so the decisions are made per site with the per-site
+            // keying (domain SITE: word k decides bond k, the top bit of word 3 is the cluster draw).  The 32
+            // threads of a warp own 32 rows that follow each other in y; they take these rows one at a time
+            // with lane = x, from the last to the first, so that the row done before is the +y neighbour
+            // (its projections are still in registers); +x comes by shuffle, +z is computed again from the
+            // neighbour's spin.  Three ballots turn the decisions of a row into its bond masks, which the
+            // thread that owns the row keeps.
+            Bx = By = 0u;
+            const uint32_t gxl = x0 + (uint32_t)lane;
+            const uint32_t rowbase0 = g0 - L * (uint32_t)lane - (DIM == 2 ? 0u : 0u);   // row of lane 0 of this warp (same z)
+            auto proj = [&](uint32_t gsite) -> float {           // XY: a = r . s;  clock: class word (u | sign << 16) as float bits
+                if (MODEL == XY) {
+                    float sn, cs;
+                    sincosf(((const float *)p.spins)[gsite], &sn, &cs);
+                    return p.rx * cs + p.ry * sn;
+                } else {
+                    int k = 2 * (int)((const uint16_t *)p.spins)[gsite] - p.mirror;
+                    if (k < 0) k += 2 * p.q;
+                    const int u = k >= p.q ? k - p.q : k;
+                    return __uint_as_float((uint32_t)u | (u == 0 ? 0u : (k >= p.q ? 2u : 1u) << 16));
+                }
+            };
+            auto decide = [&](float a, float b, uint32_t word) -> bool {
+                if (MODEL == XY) {
+                    const float pr = a * b;
+                    return pr > 0.f && (float)(word >> 8) * 5.9604644775390625e-8f < -expm1f(p.m2beta * pr);
+                } else {
+                    const uint32_t ca = __float_as_uint(a), cb = __float_as_uint(b);
+                    if (((ca & cb) >> 16) == 0u) return false;        // different sign, or one component is zero
+                    return word < __ldg(p.clock_T + (ca & 0xffffu) * (uint32_t)p.q + (cb & 0xffffu));
+                }
+            };
+            // the row above the warp's last row (periodic; 2D: the next rows of the tile or its +y halo)
+            uint32_t gup = rowbase0 + 32u * L;
+            {
+                const uint32_t gy = y0 + (uint32_t)(ly - lane) + 32u;      // y of that row
+                if (gy >= L) gup -= L * L;                                  // wrapped: back by L rows
+            }
+            float aprev = proj(gxl + gup);
+#pragma unroll 1
+            for (int yy = 31; yy >= 0; --yy) {
+                const uint32_t grow_ = rowbase0 + L * (uint32_t)yy;
+                const uint32_t site = gxl + grow_;
+                const float a = proj(site);
+                float ax = __shfl_down_sync(FULL, a, 1);
+                if (lane == 31) ax = proj(xh + grow_);
+                const uint4 w = philox4x32_10(site, t_lo, t_hi, DOM_SITE, p.k0, p.k1);
+                const uint32_t mx = __ballot_sync(FULL, decide(a, ax, w.x));
+                const uint32_t my = __ballot_sync(FULL, decide(a, aprev, w.y));
+                uint32_t mz = 0u;
+                if (DIM == 3) {
+                    const uint32_t gzn = (z0 + (uint32_t)lz + 1u == L) ? site - LL * (L - 1u) : site + LL;
+                    mz = __ballot_sync(FULL, decide(a, proj(gzn), w.z));
+                }
+                const uint32_t md = __ballot_sync(FULL, (w.w >> 31) != 0u);
+                if (lane == yy) { Bx = mx; By = my; Bz = mz; D = md; }
+                aprev = a;
+            }
+        } else {
         uint32_t ex, ey, ez = 0u;
         if (MODEL == ISING) {
             const uint32_t nxb = sp[xh + g0] >> 7;             // sign of the +x neighbour of site 31
@@ -311,9 +380,10 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 ez = eq32(own, oth);
             }
         }
-        uint32_t X[3], D;
+        uint32_t X[3];
         group_decisions<DIM>(p, (x0 + g0) >> 5, t_lo, t_hi, X, D);
-        uint32_t Bx = ex & X[0], By = ey & X[1], Bz = (DIM == 3) ? (ez & X[2]) : 0u;
+        Bx = ex & X[0]; By = ey & X[1]; Bz = (DIM == 3) ? (ez & X[2]) : 0u;
+        }
         if (p.bonds) {   // canonical bond bytes on request (parity tests): bit k = bond in direction k
 #pragma unroll
             for (int j = 0; j < 8; ++j)
@@ -334,7 +404,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
         bx_s[row] = Bx;
         pm_s[row] = By;
         if (DIM == 3) pm_s[NROWS + row] = Bz;
-        if (MODEL == ISING) {
+        if (MODEL != POTTS) {
             dr_s[row] = D;
         } else {
             // Potts: the draw word of site b of the group is W_G[128 + b] (reading 6): call 32 + b / 4, word
@@ -565,10 +635,17 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
         for (int row = warp; row < NROWS; row += NW) {
             const uint32_t st = run_start(bx_s[row], below);
             uint32_t v = lds_u16(lab_sa + (uint32_t)row * 64u + 2u * st);
+            if (SW_ROW_JUMPS > 0) {
+                // first ancestor; if it is the run start itself the run start is a root and the site is done
+                // (no further loads: fewer shared-memory wavefronts; 45 % of the run starts are roots)
+                const uint32_t v0 = v;
+                v = lds_u16(lab_sa + v);
+                const uint32_t more = (v != v0) ? 1u : 0u;
 #pragma unroll
-            for (int k = 0; k < SW_ROW_JUMPS; ++k) v = lds_u16(lab_sa + v);
+                for (int k = 1; k < SW_ROW_JUMPS; ++k) lds_u16_if(v, more, lab_sa + v);
+            }
             uint32_t word;
-            if (MODEL == ISING) word = (tile_base << 1) + v + ((dr_s[row] >> lane) & 1u);   // v = 2 x local index
+            if (MODEL != POTTS) word = (tile_base << 1) + v + ((dr_s[row] >> lane) & 1u);   // v = 2 x local index
             else word = ((tile_base + (v >> 1)) << db) | reinterpret_cast<const uint8_t *>(dr_s)[row * 32 + lane];
             p.labels[tile_base + (uint32_t)row * 32u + (uint32_t)lane] = word;
         }

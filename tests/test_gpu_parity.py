@@ -157,12 +157,17 @@ def test_tile_menu_3d(tile, rows, model, q, T, monkeypatch):
         _compare_step(g, o, f"tile {tile} R={rows} model {model} t={t}")
 
 
-@pytest.mark.parametrize("dim,L,tile", [(2, 256, "32x32"), (2, 256, "64x64"), (2, 256, "128x32"), (2, 256, "128x64"),
-                                        (3, 64, "32x8x8"), (3, 64, "32x16x8"), (3, 64, "32x16x16"), (3, 64, "64x8x8")])
+@pytest.mark.parametrize("dim,L,kernel,tile", [
+    (2, 256, "quad", "32x32"), (2, 256, "quad", "64x64"), (2, 256, "quad", "128x32"), (2, 256, "quad", "128x64"),
+    (3, 64, "quad", "32x8x8"), (3, 64, "quad", "32x16x8"), (3, 64, "quad", "32x16x16"), (3, 64, "quad", "64x8x8"),
+    (2, 512, "rows", "32x32"), (2, 512, "rows", "32x128"), (2, 512, "rows", "32x256"),
+    (3, 64, "rows", "32x32x4"), (3, 64, "rows", "32x32x8"), (3, 64, "rows", "32x32x16")])
 @pytest.mark.parametrize("model,q", [(2, 0), (3, 12)])
-def test_tile_menu_xy_clock(dim, L, tile, model, q, monkeypatch):
-    """The quad kernel's tiles for the two models that use it: XY (bond mismatch budget) and clock (bit-exact)."""
+def test_tile_menu_xy_clock(dim, L, kernel, tile, model, q, monkeypatch):
+    """XY (bond mismatch budget) and clock (bit-exact) on both bond / label kernels and all their tiles: the
+    quad kernel (default for XY) and the row kernel (default for the clock model); SW_B200_KERNEL selects."""
     sw, orc = _mods()
+    monkeypatch.setenv("SW_B200_KERNEL", kernel)
     monkeypatch.setenv("SW_B200_TILE", tile)
     T = 0.9 if dim == 2 else 2.2019
     g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=5, record_bonds=True)
