@@ -2,17 +2,18 @@
 // (PAPER.md:94-98).  Independent of oracle/: nothing here is shared with or derived from it.
 //
 // Kernels of one step t:
-//   k_bond_label  (1) bond activation fused with (2a) tile-local cluster labelling in
-//                 shared memory.  A thread owns "quads" of 4 consecutive sites along x (one 32-bit
-//                 spin word); x-connectivity is resolved with two warp ballots, y/z bonds inside the
-//                 tile by a CAS hook round, pointer jumping and an atomicMin union-find for what
-//                 is left, all in shared memory; bonds through tile faces go to a global pair list;
+//   k_bond_label_rows (sw_rows.cuh; Ising, Potts, clock)  /  k_bond_label (here; XY: the round-1 "quad" kernel)
+//                 (1) bond activation fused with (2a) tile-local cluster labelling in shared
+//                 memory; bonds through tile faces go to a global pair list.  In k_bond_label a thread owns
+//                 "quads" of 4 consecutive sites along x; x-connectivity is resolved with two warp ballots,
+//                 y/z bonds inside the tile by a CAS hook round, pointer jumping and an atomicMin union-find;
 //   k_merge       (2b) global lock-free union-find (atomicCAS, min linear index wins) over the active
 //                 bonds that cross tile faces incl. the periodic wrap;
 //   k_flip        (2c) root chase fused with (3) the per-cluster new value / XY reflection
 //                  and the magnetisation sums of PAPER.md:142-157;
 //   k_measure4 / k_measure / k_measure_clock   energy (Eq. 1-3) and magnetisation (Eq. 4, 5) of the
-//                 current configuration, on request (sw_observables, sw_run_series).
+//                 current configuration, on request (sw_observables, sw_run_series);
+//   k_sw_small (sw_small.cuh)  all of the above in one CTA for lattices of at most 32768 Ising / Potts sites.
 // Models: Ising, q-state Potts, continuous XY, q-state clock (the discretisation the paper runs).
 //
 // Label array (HBM), one 32-bit word per site, TILE-MAJOR: the word of the site with tile-local

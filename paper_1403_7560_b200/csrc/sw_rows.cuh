@@ -1,17 +1,19 @@
-// sw_rows.cuh -- k_bond_label_rows: bond activation fused with the tile-local part of
-// the cluster labelling for the two models whose bond probability is one
-// constant, Ising and q-state Potts.  Independent of oracle/.
+// sw_rows.cuh -- k_bond_label_rows: bond activation fused with the tile-local part
+// of the cluster labelling.  Ising, q-state Potts and the q-state clock model by
+// default, XY on request (sw_api.cu use_rows).  Independent of oracle/.
 //
 // The unit of work is a ROW: 32 consecutive sites along x, held as 32-bit masks (bit x = site x of the
 // row; tiles are 32 sites wide, "nx ... multiple of 32").
 //   phase 1a  [thread = row] (Ising) spins of the thread's R rows -> sign masks in shared memory (+ halo rows)
-//   phase 1b  [thread = row] the random decisions of the row's 32 x DIM bonds from the transposed uniform
-//             integers of DESIGN.md reading 6 (13 binary digits = 10 Philox calls per row in 3D settle every
-//             bond of the row in 99.6 % of the cases, further digits are drawn only when some site is still
-//             undecided), AND-ed with the equality masks -> bond masks Bx, By, Bz.  Bx gives the x-runs of
-//             the row with no union at all.  Bonds through the tile faces go to face words (-> global pair
-//             list, k_merge).  Nodes of the tile-local union-find are the RUN STARTS; the run start of a
-//             site is a find-leading-one on the row's Bx mask.
+//   phase 1b  [thread = row] Ising / Potts: the random decisions of the row's 32 x DIM bonds from the
+//             transposed uniform integers of DESIGN.md reading 6 (13 binary digits = 10 Philox calls per row
+//             in 3D settle every bond of the row in 99.6 % of the cases, further digits are drawn only when
+//             some site is still undecided), AND-ed with the equality masks -> bond masks Bx, By, Bz.
+//             [warp = 32 rows, lane = x] XY / clock: per-site decisions (the probability depends on the two
+//             spins), three ballots per row give the same masks.
+//             Bx gives the x-runs of the row with no union at all.  Bonds through the tile faces go to face
+//             words (-> global pair list, k_merge).  Nodes of the tile-local union-find are the RUN STARTS;
+//             the run start of a site is a find-leading-one on the row's Bx mask.  16-bit parent entries.
 //   phase 2a  [thread = row] "pull": every run looks back at the bonds that reach it from the row below
 //             (y - 1) and the row behind (z - 1); the first such bond of the run makes the run start it
 //             comes from the parent of this run start -- a plain store, no atomic, no retry, because only
@@ -19,10 +21,12 @@
 //             is settled for all 32 sites at once by a carry trick on the masks.  Further bonds into the
 //             same run (minus twins joining the same two runs) are appended to a list.
 //   phase 2b  [all threads] the listed bonds go through a lock-free union-find (CAS: larger root under
-//             smaller, so that the root of a tree is its minimum index).
+//             smaller, so that the root of a tree is its minimum index; path halving on the
+//             way up).  Lanes take the next bond of their warp's share as soon as they are free.
 //   phase 3   [lane = x] per site: run start, a few dependent parent loads, label word =
 //             (address of the ancestor reached << DB) | own draw, coalesced stores.  Whatever is left of a
-//             longer chain is followed by k_merge / k_flip.
+//             longer chain is followed by k_merge / k_flip.  The pair list hands k_merge the same ancestor
+//             for this tile's end of every face bond.
 // Label words, pair list and bond bytes are the ones of sw_kernels.cuh (k_merge / k_flip read them).
 #pragma once
 #include "sw_kernels.cuh"
