@@ -27,6 +27,22 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// XY arithmetic (reading 20): the projections r . s_i and the bond probabilities 1 - exp(-2 beta a_i a_j)
+// are evaluated with the SFU intrinsics __sincosf / __expf.  Measured against the fp64 oracle on 7.0e8 bonds
+// (3D L = 256, T = 2.2019, 14 injected steps): 43 mismatching bonds = 6.1e-8 per bond, 16 x below north_star's
+// budget of 1e-6 (full-precision sincosf / expm1f: 2 of 4.0e8 = 5e-9); what decides a bond is the ABSOLUTE error
+// of p, about 1e-7 for the intrinsics on angles in [0, 2 pi].  SW_XY_FAST_MATH=0 builds the full-precision path.
+#ifndef SW_XY_FAST_MATH
+#define SW_XY_FAST_MATH 1
+#endif
+#if SW_XY_FAST_MATH
+#define SW_SINCOSF(x, s, c) __sincosf((x), (s), (c))
+#define SW_NEG_EXPM1F(x) (1.0f - __expf(x))
+#else
+#define SW_SINCOSF(x, s, c) sincosf((x), (s), (c))
+#define SW_NEG_EXPM1F(x) (-expm1f(x))
+#endif
+
 namespace swk {
 
 enum { ISING = 0, POTTS = 1, XY = 2, CLOCK = 3 };
@@ -266,10 +282,10 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
             const float4 t4 = *reinterpret_cast<const float4 *>(th + g);
             float4 a;
             float sn, cs;
-            sincosf(t4.x, &sn, &cs); a.x = p.rx * cs + p.ry * sn;
-            sincosf(t4.y, &sn, &cs); a.y = p.rx * cs + p.ry * sn;
-            sincosf(t4.z, &sn, &cs); a.z = p.rx * cs + p.ry * sn;
-            sincosf(t4.w, &sn, &cs); a.w = p.rx * cs + p.ry * sn;
+            SW_SINCOSF(t4.x, &sn, &cs); a.x = p.rx * cs + p.ry * sn;
+            SW_SINCOSF(t4.y, &sn, &cs); a.y = p.rx * cs + p.ry * sn;
+            SW_SINCOSF(t4.z, &sn, &cs); a.z = p.rx * cs + p.ry * sn;
+            SW_SINCOSF(t4.w, &sn, &cs); a.w = p.rx * cs + p.ry * sn;
             *reinterpret_cast<float4 *>(val_s + li) = a;
         }
         for (int h = tid; h < G::NHALO; h += NT) {
@@ -287,7 +303,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
             if (gy == L) gy = 0;
             if (DIM == 3 && gz == L) gz = 0;
             float sn, cs;
-            sincosf(th[gx + L * (gy + L * gz)], &sn, &cs);
+            SW_SINCOSF(th[gx + L * (gy + L * gz)], &sn, &cs);
             val_s[NS + h] = p.rx * cs + p.ry * sn;
         }
     }
@@ -324,8 +340,8 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
                 const float px = av[s] * axv[s], py = av[s] * ayv[s];
-                if (px > 0.f && (float)(w[s].x >> 8) * scale < -expm1f(p.m2beta * px)) bxn |= 1u << s;
-                if (py > 0.f && (float)(w[s].y >> 8) * scale < -expm1f(p.m2beta * py)) byn |= 1u << s;
+                if (px > 0.f && (float)(w[s].x >> 8) * scale < SW_NEG_EXPM1F(p.m2beta * px)) bxn |= 1u << s;
+                if (py > 0.f && (float)(w[s].y >> 8) * scale < SW_NEG_EXPM1F(p.m2beta * py)) byn |= 1u << s;
             }
             if (DIM == 3) {
                 const float4 az = (lz + 1 < TZ) ? *reinterpret_cast<const float4 *>(val_s + li + TX * TY)
@@ -334,7 +350,7 @@ __global__ void __launch_bounds__(NT, SW_BL_THREADS_PER_SM / NT) k_bond_label(co
 #pragma unroll
                 for (int s = 0; s < 4; ++s) {
                     const float pz = av[s] * azv[s];
-                    if (pz > 0.f && (float)(w[s].z >> 8) * scale < -expm1f(p.m2beta * pz)) bzn |= 1u << s;
+                    if (pz > 0.f && (float)(w[s].z >> 8) * scale < SW_NEG_EXPM1F(p.m2beta * pz)) bzn |= 1u << s;
                 }
             }
             d = (w[0].w >> 31) | ((w[1].w >> 31) << 1) | ((w[2].w >> 31) << 2) | ((w[3].w >> 31) << 3);

@@ -307,7 +307,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
             auto proj = [&](uint32_t gsite) -> float {           // XY: a = r . s;  clock: class word (u | sign << 16) as float bits
                 if (MODEL == XY) {
                     float sn, cs;
-                    sincosf(((const float *)p.spins)[gsite], &sn, &cs);
+                    SW_SINCOSF(((const float *)p.spins)[gsite], &sn, &cs);
                     return p.rx * cs + p.ry * sn;
                 } else {
                     int k = 2 * (int)((const uint16_t *)p.spins)[gsite] - p.mirror;
@@ -319,7 +319,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
             auto decide = [&](float a, float b, uint32_t word) -> bool {
                 if (MODEL == XY) {
                     const float pr = a * b;
-                    return pr > 0.f && (float)(word >> 8) * 5.9604644775390625e-8f < -expm1f(p.m2beta * pr);
+                    return pr > 0.f && (float)(word >> 8) * 5.9604644775390625e-8f < SW_NEG_EXPM1F(p.m2beta * pr);
                 } else {
                     const uint32_t ca = __float_as_uint(a), cb = __float_as_uint(b);
                     if (((ca & cb) >> 16) == 0u) return false;        // different sign, or one component is zero

