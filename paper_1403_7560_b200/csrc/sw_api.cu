@@ -339,9 +339,9 @@ template <int DIM, int MODEL>
 void launch_measure_dm(sw_ctx *c, bool with_m)
 {
     if (MODEL == XY) {
-        const unsigned g = (unsigned)(c->N / 256);
-        if (with_m) k_measure<DIM, MODEL, true><<<g, 256, 0, c->stream>>>(c->p);
-        else k_measure<DIM, MODEL, false><<<g, 256, 0, c->stream>>>(c->p);
+        const unsigned g = (unsigned)(c->N / 1024);  // four sites per thread
+        if (with_m) k_measure_xy<DIM, true><<<g, 256, 0, c->stream>>>(c->p);
+        else k_measure_xy<DIM, false><<<g, 256, 0, c->stream>>>(c->p);
     } else {
         const unsigned g = (unsigned)(c->N / 1024);  // four sites per thread
         if (with_m) k_measure4<DIM, MODEL, true><<<g, 256, 0, c->stream>>>(c->p);
@@ -352,7 +352,8 @@ void launch_measure_dm(sw_ctx *c, bool with_m)
 void launch_measure(sw_ctx *c, bool with_m)
 {
     if (c->model == SW_CLOCK) {
-        const unsigned g = (unsigned)(c->N / 256);
+        unsigned g = (unsigned)(c->N / 256);
+        if (g > 148u * 8u) g = 148u * 8u;   // a CTA flushes its histograms once: few CTAs, many sites each
         if (c->dim == 2) k_measure_clock<2><<<g, 256, 0, c->stream>>>(c->p);
         else k_measure_clock<3><<<g, 256, 0, c->stream>>>(c->p);
         return;

@@ -11,7 +11,7 @@
 //                 bonds that cross tile faces incl. the periodic wrap;
 //   k_flip        (2c) root chase fused with (3) the per-cluster new value / XY reflection
 //                  and the magnetisation sums of PAPER.md:142-157;
-//   k_measure4 / k_measure / k_measure_clock   energy (Eq. 1-3) and magnetisation (Eq. 4, 5) of the
+//   k_measure4 / k_measure_xy / k_measure_clock   energy (Eq. 1-3) and magnetisation (Eq. 4, 5) of the
 //                 current configuration, on request (sw_observables, sw_run_series);
 //   k_sw_small (sw_small.cuh)  all of the above in one CTA for lattices of at most 32768 Ising / Potts sites.
 // Models: Ising, q-state Potts, continuous XY, q-state clock (the discretisation the paper runs).
@@ -919,80 +919,56 @@ __global__ void __launch_bounds__(256) k_export_labels(const Params p)
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_measure: E (Eq. 1-3) and, if WITH_M, the magnetisation sums (Eq. 4, 5) of the configuration.
-// One thread per site, its d owned bonds; block reduction, one atomic per CTA and quantity.
+// k_measure_xy: E = -sum cos(theta_i - theta_j) (Eq. 3) and, if WITH_M, (sum cos, sum sin), four consecutive
+// sites per thread.  The 12 (8) cosines of a thread and the sums of a warp are accumulated in fp32 (a few
+// hundred terms of magnitude <= 1: rounding error ~1e-5 per warp sum, random in sign), the warp sums in
+// fp64: the fp64 pipe of this GPU is slow, and one thread per site with fp64 shuffles made this pass cost
+// as much as the whole SW step.
 // ------------------------------------------------------------------------------------------------
-template <int DIM, int MODEL, bool WITH_M>
-__global__ void __launch_bounds__(256) k_measure(const Params p)
+template <int DIM, bool WITH_M>
+__global__ void __launch_bounds__(256) k_measure_xy(const Params p)
 {
-    __shared__ unsigned long long hist_s[256];
     __shared__ double red_s[3][8];
-    __shared__ long long redi_s[2][8];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t i = blockIdx.x * 256u + tid;  // N is a multiple of 1024
-    const uint32_t L = p.L;
-    if (MODEL == POTTS && WITH_M) {
-        hist_s[tid] = 0ull;
-        __syncthreads();
-    }
+    const uint32_t L = p.L, LL = L * L;
+    const uint32_t g = (blockIdx.x * 256u + tid) * 4u;  // N is a multiple of 1024
     uint32_t x, y, z;
-    decode(p, i, x, y, z);
-    const uint32_t jx = (x + 1 == L) ? i - (L - 1) : i + 1;
-    const uint32_t jy = (y + 1 == L) ? i - L * (L - 1) : i + L;
-    const uint32_t jz = (DIM == 3) ? ((z + 1 == L) ? i - L * L * (L - 1) : i + L * L) : 0u;
-    long long e = 0, m = 0;
-    double ex = 0.0, cx = 0.0, cy = 0.0;
-    if (MODEL == ISING) {
-        const int8_t *s = (const int8_t *)p.spins;
-        const int v = s[i];
-        e = -(v * s[jx] + v * s[jy] + (DIM == 3 ? v * s[jz] : 0));
-        m = v;
-    } else if (MODEL == POTTS) {
-        const uint8_t *s = (const uint8_t *)p.spins;
-        const uint32_t v = s[i];
-        e = (v != s[jx]) + (v != s[jy]) + (DIM == 3 ? (v != s[jz]) : 0);
-        if (WITH_M) atomicAdd(&hist_s[v], 1ull);
-    } else {
-        const float *s = (const float *)p.spins;
-        const float v = s[i];
-        ex = -((double)cosf(v - s[jx]) + (double)cosf(v - s[jy]) + (DIM == 3 ? (double)cosf(v - s[jz]) : 0.0));
-        if (WITH_M) {
-            float sn, cs;
-            sincosf(v, &sn, &cs);
-            cx = cs; cy = sn;
-        }
+    decode(p, g, x, y, z);
+    const float *s = (const float *)p.spins;
+    const float4 a = *reinterpret_cast<const float4 *>(s + g);
+    const float ax = s[(x + 4 == L) ? g + 4 - L : g + 4];
+    const float4 b = *reinterpret_cast<const float4 *>(s + ((y + 1 == L) ? g - L * (L - 1) : g + L));
+    float e = cosf(a.x - a.y) + cosf(a.y - a.z) + cosf(a.z - a.w) + cosf(a.w - ax)
+            + cosf(a.x - b.x) + cosf(a.y - b.y) + cosf(a.z - b.z) + cosf(a.w - b.w);
+    if (DIM == 3) {
+        const float4 c = *reinterpret_cast<const float4 *>(s + ((z + 1 == L) ? g - LL * (L - 1) : g + LL));
+        e += cosf(a.x - c.x) + cosf(a.y - c.y) + cosf(a.z - c.z) + cosf(a.w - c.w);
     }
-    if (MODEL == XY) {
-        for (int o = 16; o > 0; o >>= 1) {
-            ex += __shfl_down_sync(FULL, ex, o);
-            cx += __shfl_down_sync(FULL, cx, o);
-            cy += __shfl_down_sync(FULL, cy, o);
-        }
-        if (lane == 0) { red_s[0][warp] = ex; red_s[1][warp] = cx; red_s[2][warp] = cy; }
-        __syncthreads();
-        if (tid == 0) {
-            for (int w = 1; w < 8; ++w) { ex += red_s[0][w]; cx += red_s[1][w]; cy += red_s[2][w]; }
-            atomicAdd(&p.acc->E_xy, ex);
-            if (WITH_M) { atomicAdd(&p.acc->mx, cx); atomicAdd(&p.acc->my, cy); }
-        }
-    } else {
-        int ei = __reduce_add_sync(FULL, (int)e), mi = __reduce_add_sync(FULL, (int)m);
-        if (lane == 0) { redi_s[0][warp] = ei; redi_s[1][warp] = mi; }
-        __syncthreads();
-        if (tid == 0) {
-            long long es = 0, ms = 0;
-            for (int w = 0; w < 8; ++w) { es += redi_s[0][w]; ms += redi_s[1][w]; }
-            atomicAdd(&p.acc->E_int, (unsigned long long)es);
-            if (WITH_M && MODEL == ISING) atomicAdd(&p.acc->M_int, (unsigned long long)ms);
-        }
-        if (MODEL == POTTS && WITH_M) {
-            if (tid < p.q && hist_s[tid]) atomicAdd(&p.acc->nk[tid], hist_s[tid]);
-        }
+    e = -e;
+    float cx = 0.f, cy = 0.f;
+    if (WITH_M) {
+        float sn, cs;
+        sincosf(a.x, &sn, &cs); cx += cs; cy += sn;
+        sincosf(a.y, &sn, &cs); cx += cs; cy += sn;
+        sincosf(a.z, &sn, &cs); cx += cs; cy += sn;
+        sincosf(a.w, &sn, &cs); cx += cs; cy += sn;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        e += __shfl_down_sync(FULL, e, o);
+        if (WITH_M) { cx += __shfl_down_sync(FULL, cx, o); cy += __shfl_down_sync(FULL, cy, o); }
+    }
+    if (lane == 0) { red_s[0][warp] = (double)e; red_s[1][warp] = (double)cx; red_s[2][warp] = (double)cy; }
+    __syncthreads();
+    if (tid == 0) {
+        double es = 0.0, xs = 0.0, ys = 0.0;
+        for (int w = 0; w < 8; ++w) { es += red_s[0][w]; xs += red_s[1][w]; ys += red_s[2][w]; }
+        atomicAdd(&p.acc->E_xy, es);
+        if (WITH_M) { atomicAdd(&p.acc->mx, xs); atomicAdd(&p.acc->my, ys); }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_measure4 (Ising, Potts): as k_measure, four consecutive sites per thread.  The spin words of the
+// k_measure4 (Ising, Potts): E (Eq. 1, 2) and, if WITH_M, the magnetisation sums (Eq. 4, 5); four consecutive sites per thread.  The spin words of the
 // quad and of its +x / +y / +z neighbours give byte-equality masks; with spins in the model's range
 // the energy is a popcount: Ising -sum s_i s_j = (#pairs - 2 #equal), Potts #unequal pairs.
 // ------------------------------------------------------------------------------------------------
@@ -1059,7 +1035,7 @@ __global__ void __launch_bounds__(256) k_measure4(const Params p)
 // ------------------------------------------------------------------------------------------------
 // k_measure_clock: the exact integer histograms of the clock model -- n[p] (sites per state, the
 // paper's fmy[] table gives M from it) and D[d] (nearest-neighbour pairs per state difference, the
-// paper's rule[] table gives E from it).  One site per thread, shared histograms.
+// paper's rule[] table gives E from it).  Shared histograms per CTA, grid-stride over the sites.
 // ------------------------------------------------------------------------------------------------
 template <int DIM>
 __global__ void __launch_bounds__(256) k_measure_clock(const Params p)
@@ -1068,25 +1044,29 @@ __global__ void __launch_bounds__(256) k_measure_clock(const Params p)
     const int tid = threadIdx.x;
     for (int k = tid; k < 512; k += 256) { n_s[k] = 0u; d_s[k] = 0u; }
     __syncthreads();
-    const uint32_t i = blockIdx.x * 256u + tid;  // N is a multiple of 1024
+    // grid-stride over the sites: a CTA keeps its shared histograms for many sites and adds them to the
+    // global ones once (one CTA per 256 sites made the 2 q global atomics of every CTA the whole cost)
     const uint32_t L = p.L;
-    uint32_t x, y, z;
-    decode(p, i, x, y, z);
     const uint16_t *s = (const uint16_t *)p.spins;
-    const int q = p.q, v = s[i];
-    atomicAdd(&n_s[v], 1u);
-    const uint32_t jx = (x + 1 == L) ? i - (L - 1) : i + 1;
-    const uint32_t jy = (y + 1 == L) ? i - L * (L - 1) : i + L;
-    int dx = v - (int)s[jx], dy = v - (int)s[jy];
-    if (dx < 0) dx += q;
-    if (dy < 0) dy += q;
-    atomicAdd(&d_s[dx], 1u);
-    atomicAdd(&d_s[dy], 1u);
-    if (DIM == 3) {
-        const uint32_t jz = (z + 1 == L) ? i - L * L * (L - 1) : i + L * L;
-        int dz = v - (int)s[jz];
-        if (dz < 0) dz += q;
-        atomicAdd(&d_s[dz], 1u);
+    const int q = p.q;
+    for (uint32_t i = blockIdx.x * 256u + tid; i < p.N; i += gridDim.x * 256u) {  // N is a multiple of 1024
+        uint32_t x, y, z;
+        decode(p, i, x, y, z);
+        const int v = s[i];
+        atomicAdd(&n_s[v], 1u);
+        const uint32_t jx = (x + 1 == L) ? i - (L - 1) : i + 1;
+        const uint32_t jy = (y + 1 == L) ? i - L * (L - 1) : i + L;
+        int dx = v - (int)s[jx], dy = v - (int)s[jy];
+        if (dx < 0) dx += q;
+        if (dy < 0) dy += q;
+        atomicAdd(&d_s[dx], 1u);
+        atomicAdd(&d_s[dy], 1u);
+        if (DIM == 3) {
+            const uint32_t jz = (z + 1 == L) ? i - L * L * (L - 1) : i + L * L;
+            int dz = v - (int)s[jz];
+            if (dz < 0) dz += q;
+            atomicAdd(&d_s[dz], 1u);
+        }
     }
     __syncthreads();
     for (int k = tid; k < q; k += 256) {
