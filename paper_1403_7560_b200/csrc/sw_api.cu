@@ -149,17 +149,16 @@ bool pick_ops(int dim, int tx, int ty, int tz, TileOps &o)
     return false;
 }
 
-// Which bond / label kernel a model runs: Ising and Potts always the row kernel (sw_rows.cuh); the clock
-// model the row kernel by default, XY the quad kernel by default (measured: the row kernel has to compute
-// the projection of the +z neighbour a second time, which costs XY more than the cheaper labelling saves:
-// C5 0.341 vs 0.286 ms per step; clock X3 0.249 vs 0.260).  SW_B200_KERNEL=rows|quad forces one of them.
+// Which bond / label kernel a model runs: the row kernel (sw_rows.cuh) for every model; the quad kernel of
+// round 1 (sw_kernels.cuh k_bond_label) stays selectable for XY and the clock model with SW_B200_KERNEL=quad.
+// Measured (ms per step, rows vs quad): clock X3 0.249 vs 0.260; XY with the SFU intrinsics C5 0.245 vs
+// 0.247, X2 0.080 vs 0.084 (with full-precision sincosf the row kernel lost on XY, 0.341 vs 0.286: it computes
+// the projection of the +z neighbour a second time).
 bool use_rows(int model)
 {
     if (model == SW_ISING || model == SW_POTTS) return true;
     const char *kern = std::getenv("SW_B200_KERNEL");
-    if (kern && std::strcmp(kern, "quad") == 0) return false;
-    if (kern && std::strcmp(kern, "rows") == 0) return true;
-    return model == SW_CLOCK;
+    return !(kern && std::strcmp(kern, "quad") == 0);
 }
 
 // Small lattices (fewer tiles than the GPU has room for): what counts is the critical path of one CTA,
