@@ -135,6 +135,25 @@ int sw_get_labels(sw_ctx *c, uint32_t *host_dst, size_t bytes);
  * representation; Potts with Eq. (5)'s normalisation).  Either pointer may be NULL. */
 int sw_get_cluster_stats(sw_ctx *c, uint64_t *host_n_clusters, uint64_t *host_sum_nc2);
 
+/* The same two sums for callers that must not allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): no cudaMalloc / cudaFree, no allocating
+ * library routine, no host synchronisation, no context.
+ *   device_labels  DEVICE pointer, n uint32 canonical labels as sw_get_labels returns them: the label of
+ *                  a site is the index (< n) of one site of its cluster, the same for all its sites
+ *                  (a label >= n is skipped); read only, owned by the caller;
+ *   n              number of sites, 1 .. SW_STATIC_MAX_SITES; anything else returns SW_EINVAL with the
+ *                  limit in sw_last_error() and launches nothing;
+ *   device_out     DEVICE pointer to two uint64, 8-byte aligned, owned by the caller: [0] = number of
+ *                  clusters, [1] = sum_c n_c^2; written asynchronously on the stream;
+ *   cuda_stream    cudaStream_t passed as void * (NULL = the legacy default stream) of the CURRENT device.
+ * The per-site size counters (scratch) live in a static device array of SW_STATIC_MAX_SITES uint32
+ * (4 MiB) inside the library, which every GPU that loads the library holds until the process exits.
+ * All calls share that array and it keeps the last call's counters: every call clears the part it
+ * uses first, and two calls that overlap on the GPU (different streams or threads) race -- order them
+ * on one stream or with events. */
+#define SW_STATIC_MAX_SITES (1u << 20)
+int sw_cluster_stats_static(const uint32_t *device_labels, size_t n, uint64_t *device_out, void *cuda_stream);
+
 /* Exact integer sums of the current configuration.  Ising: *host_E = -sum s_i s_j,
  * host_M_or_nk[0] = sum s_i (n >= 1).  Potts: *host_E = #unequal pairs, host_M_or_nk[k] = n_k for
  * k < min(n, q).  SW_EINVAL for XY. */

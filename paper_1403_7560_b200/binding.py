@@ -65,6 +65,7 @@ def lib():
     L.sw_info.argtypes = [vp, i32]
     L.sw_info.restype = C.c_longlong
     L.sw_micro_bench.argtypes = [i32, sz, sz, i32, C.POINTER(dbl)]
+    L.sw_cluster_stats_static.argtypes = [vp, sz, vp, vp]
     _lib = L
     return _lib
 
@@ -97,6 +98,19 @@ def micro_bench(kind, n, table_words=0, reps=10):
 
 def dbl_():
     return C.c_double()
+
+
+STATIC_MAX_SITES = 1 << 20   # SW_STATIC_MAX_SITES (include/sw.h)
+
+
+def cluster_stats_static(device_labels, n, device_out, cuda_stream=0):
+    """sw_cluster_stats_static (include/sw.h): number of clusters and sum of squared cluster sizes of n
+    canonical labels, with the scratch counters in the library's static device array -- the call
+    allocates nothing.  device_labels / device_out are DEVICE addresses (ints, e.g. tensor.data_ptr()) of
+    n uint32 / two uint64; cuda_stream a cudaStream_t as int (0 = the legacy default stream).
+    Asynchronous; calls share the scratch array, so calls that overlap on the GPU race."""
+    _check(lib().sw_cluster_stats_static(C.c_void_p(int(device_labels)), int(n), C.c_void_p(int(device_out)),
+                                         C.c_void_p(int(cuda_stream))))
 
 
 class SwendsenWang:

@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1136,3 +1137,94 @@ int sw_philox_selftest(const uint32_t *ctr, const uint32_t *key, uint32_t *out, 
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// sw_cluster_stats_static (include/sw.h): cluster statistics with NO device allocation.  The size
+// counters that sw_get_cluster_stats takes from cudaMalloc live in the file-scope device array below
+// (SW_STATIC_MAX_SITES counters = 4 MiB, held by every GPU that loads the library until exit).
+// In host code the array's name `g_static_sizes` is a host-side stand-in, not a device address: the
+// address the kernels get comes from cudaGetSymbolAddress, asked once per device with that device
+// current.  Every call shares the array and leaves its counters in it: a call clears the part it uses
+// first, and calls that overlap on the GPU (two streams, two threads) race.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) uint32_t g_static_sizes[SW_STATIC_MAX_SITES];
+
+namespace {
+
+constexpr int STATIC_MAX_DEVICES = 64;
+uint32_t *g_static_ptr[STATIC_MAX_DEVICES];   // device address of g_static_sizes on device d, or NULL
+std::mutex g_static_mutex;
+
+// counters of this call and the two outputs start at zero
+__global__ void __launch_bounds__(256) k_static_clear(uint32_t *sizes, uint32_t n, unsigned long long *out)
+{
+    const uint32_t i = blockIdx.x * 256u + threadIdx.x;
+    if (i < n) sizes[i] = 0u;
+    if (i < 2u) out[i] = 0ull;
+}
+
+// the variant of k_cluster_sizes for canonical labels (sw_get_labels: label = a site index of the
+// cluster, the same for all its sites): every site adds 1 to the counter of its label
+__global__ void __launch_bounds__(256) k_static_cluster_sizes(const uint32_t *__restrict__ labels, uint32_t n, uint32_t *sizes)
+{
+    const uint32_t i = blockIdx.x * 256u + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t a = labels[i];
+    if (a < n) atomicAdd(&sizes[a], 1u);   // (a label outside the lattice is skipped, never written through)
+}
+
+// as k_cluster_moments, with a bound for ragged n
+__global__ void __launch_bounds__(256) k_static_cluster_moments(const uint32_t *sizes, uint32_t n, unsigned long long *out)
+{
+    const uint32_t a = blockIdx.x * 256u + threadIdx.x;
+    const unsigned long long c = a < n ? sizes[a] : 0u;
+    unsigned long long cnt = c ? 1ull : 0ull, sq = c * c;
+    for (int o = 16; o > 0; o >>= 1) {
+        cnt += __shfl_down_sync(FULL, cnt, o);
+        sq += __shfl_down_sync(FULL, sq, o);
+    }
+    if ((threadIdx.x & 31) == 0 && cnt) { atomicAdd(&out[0], cnt); atomicAdd(&out[1], sq); }
+}
+
+// set-up, once per device, with that device current
+int static_scratch(uint32_t **ptr)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SW_ECUDA, "sw_cluster_stats_static: no usable CUDA device (this library has no CPU fallback)"); }
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(SW_EINVAL, "sw_cluster_stats_static: device ordinal out of range");
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        uint32_t *q = nullptr;
+        e = cudaGetSymbolAddress((void **)&q, g_static_sizes);
+        if (e != cudaSuccess || !q) {
+            cudaGetLastError();
+            return fail(SW_ECUDA, std::string("sw_cluster_stats_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+        }
+        g_static_ptr[dev] = q;
+    }
+    *ptr = g_static_ptr[dev];
+    return SW_OK;
+}
+
+}  // namespace
+
+extern "C" int sw_cluster_stats_static(const uint32_t *device_labels, size_t n, uint64_t *device_out, void *cuda_stream)
+{
+    if (!device_labels || !device_out) return fail(SW_EINVAL, "sw_cluster_stats_static: NULL pointer");
+    if (n == 0 || n > (size_t)SW_STATIC_MAX_SITES)
+        return fail(SW_EINVAL, "sw_cluster_stats_static: n must be 1.." + std::to_string((size_t)SW_STATIC_MAX_SITES) +
+                               " sites (SW_STATIC_MAX_SITES: the static scratch array holds one counter per site); got " + std::to_string(n));
+    uint32_t *sizes = nullptr;
+    const int rc = static_scratch(&sizes);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const unsigned g = (unsigned)((n + 255) / 256);
+    unsigned long long *out = reinterpret_cast<unsigned long long *>(device_out);
+    k_static_clear<<<g, 256, 0, st>>>(sizes, (uint32_t)n, out);
+    k_static_cluster_sizes<<<g, 256, 0, st>>>(device_labels, (uint32_t)n, sizes);
+    k_static_cluster_moments<<<g, 256, 0, st>>>(sizes, (uint32_t)n, out);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "sw_cluster_stats_static");
+    return SW_OK;
+}
