@@ -85,7 +85,7 @@ bool pick_ops_rows(int dim, int tx, int ty, int tz, int rows, TileOps &o)
 #define SW_EXP_FLIP_QPT 8
 #endif
     if (MODEL != ISING) return false;
-    if (dim == 3 && ty == 32 && tz == 16) { o = make_ops_rows<3, ISING, 32, 16, 1, SW_EXP_FLIP_QPT, 3>(); return true; }
+    if (dim == 3 && ty == 32 && tz == 16) { o = make_ops_rows<3, ISING, 32, 16, 1, SW_EXP_FLIP_QPT, 4>(); return true; }
     if (dim == 2 && ty == 128) { o = make_ops_rows<2, ISING, 128, 1, 1, 4, 12>(); return true; }
     return false;
 #else
@@ -101,7 +101,7 @@ bool pick_ops_rows(int dim, int tx, int ty, int tz, int rows, TileOps &o)
     SW_ROWS3(4, 1, 4, 12)
     SW_ROWS3(8, 1, 4, 6)
     SW_ROWS3(8, 2, 4, 6)
-    SW_ROWS3(16, 1, 8, 3)
+    SW_ROWS3(16, 1, 8, (MODEL == ISING ? 4 : 3))   // Ising: 32 registers and 54.8 KB per CTA, four CTAs per SM
     SW_ROWS3(16, 2, 8, 3)
 #undef SW_ROWS2
 #undef SW_ROWS3
@@ -550,6 +550,12 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     };
     e = cudaFuncSetAttribute(c->ops.bond_label, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ops.smem_bond_label);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_bond_label)");
+    if (model == SW_ISING || model == SW_POTTS) {
+        // all of the SM's shared memory for the CTAs of the bond / label kernel (four CTAs of 54.8 KB for the 3D Ising
+        // tile); XY and clock keep the default split: their threshold-table reads live on L1
+        e = cudaFuncSetAttribute(c->ops.bond_label, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+        if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_bond_label, carveout)");
+    }
     if (c->small) {
         e = cudaFuncSetAttribute(c->small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->small_smem);
         if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_sw_small)");
