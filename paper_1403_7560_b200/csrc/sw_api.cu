@@ -122,7 +122,7 @@ bool pick_ops_rows1(int dim, int tx, int ty, int tz, TileOps &o)
     if (dim == 2 && ty == 256) { o = make_ops_rows<2, MODEL, 256, 1, 1, 4, 6>(); return true; }
     if (dim == 3 && ty == 32 && tz == 4) { o = make_ops_rows<3, MODEL, 32, 4, 1, 4, 12>(); return true; }
     if (dim == 3 && ty == 32 && tz == 8) { o = make_ops_rows<3, MODEL, 32, 8, 1, 4, 6>(); return true; }
-    if (dim == 3 && ty == 32 && tz == 16) { o = make_ops_rows<3, MODEL, 32, 16, 1, 8, 3>(); return true; }
+    if (dim == 3 && ty == 32 && tz == 16) { o = make_ops_rows<3, MODEL, 32, 16, 1, 8, (MODEL == XY ? 4 : 3)>(); return true; }
     return false;
 #endif
 }
@@ -550,9 +550,9 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     };
     e = cudaFuncSetAttribute(c->ops.bond_label, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ops.smem_bond_label);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_bond_label)");
-    if (model == SW_ISING || model == SW_POTTS) {
-        // all of the SM's shared memory for the CTAs of the bond / label kernel (four CTAs of 54.8 KB for the 3D Ising
-        // tile); XY and clock keep the default split: their threshold-table reads live on L1
+    if (model == SW_ISING || model == SW_POTTS || model == SW_XY) {
+        // all of the SM's shared memory for the CTAs of the bond / label kernel (four CTAs of 54.7 KB for the 3D Ising
+        // and XY tiles); the clock model keeps the default split: its threshold-table reads live on L1
         e = cudaFuncSetAttribute(c->ops.bond_label, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_bond_label, carveout)");
     }

@@ -64,8 +64,8 @@ struct RowGeom {
     static constexpr int OFF_FACE = OFF_SG + (NSG + 3) / 4 * 4;
     static constexpr int OFF_FPRE = OFF_FACE + NFWP;     // NFW prefix counts, [NFWP] = base in the pair list, [NFWP+1] = list length, [NFWP+2] = its valid part
     static constexpr int OFF_LIST = OFF_FPRE + NFWP + 4; // bonds left for the union-find: (node a << 16) | node b
-    // (the 3D Ising tile of 16 planes keeps a sixth: 54.8 KB per CTA, so that four CTAs of 512 threads fit one SM)
-    static constexpr int LIST_CAP = (DIM == 3 && TZ == 16 && MODEL == ISING) ? NS / 6 : NS / 4;
+    // (the 3D Ising and XY tiles of 16 planes keep a sixth: 54.7 KB per CTA, so that four CTAs of 512 threads fit one SM)
+    static constexpr int LIST_CAP = (DIM == 3 && TZ == 16 && (MODEL == ISING || MODEL == XY)) ? NS / 6 : NS / 4;
     static constexpr int WORDS = OFF_LIST + LIST_CAP;
     static constexpr size_t smem_bytes = (size_t)WORDS * 4;
 };
