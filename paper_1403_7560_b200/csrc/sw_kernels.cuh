@@ -768,6 +768,15 @@ __global__ void __launch_bounds__(NT, (SW_FLIP_THREADS_PER_SM / NT > 0 ? SW_FLIP
     int m_loc = 0;
     uint32_t cnt_lo = 0u, cnt_hi = 0u;  // Potts, q <= 8: per-thread counts of states 0-3 / 4-7, one byte each
     unsigned chase_hops = 0;
+    constexpr int STEP = NT * 4;                                                     // sites between two quads of a thread
+    constexpr int STEP_PLANES = (DIM == 3 && STEP % (TX * TY) == 0) ? STEP / (TX * TY) : 0;
+    constexpr int STEP_ROWS = (DIM == 2 && STEP % TX == 0) ? STEP / TX : 0;
+    uint32_t g_first, g_step;
+    {
+        const int li0 = tid * 4, lx = li0 % TX, ly = (li0 / TX) % TY, lz = li0 / (TX * TY);
+        g_first = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
+        g_step = STEP_PLANES > 0 ? (uint32_t)STEP_PLANES * L * L : (uint32_t)STEP_ROWS * L;
+    }
     // the label words of the NEXT quad are requested before the parents of this one are followed: the
     // kernel is bound by the latency of these reads (DRAM), not by instruction issue
 #if SW_FLIP_PREFETCH == 2
@@ -811,8 +820,14 @@ __global__ void __launch_bounds__(NT, (SW_FLIP_THREADS_PER_SM / NT > 0 ? SW_FLIP
         }
         __syncwarp();
 
-        const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
-        const uint32_t g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
+        // linear index of the quad's first site: the quads of a thread are a whole number of planes (3D) or rows (2D)
+        // apart, so one multiply-add per quad replaces the decomposition of li
+        uint32_t g;
+        if (STEP_PLANES > 0 || STEP_ROWS > 0) g = g_first + (uint32_t)j * g_step;
+        else {
+            const int lx = li % TX, ly = (li / TX) % TY, lz = li / (TX * TY);
+            g = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
+        }
         if (MODEL == ISING) {
             // "All spins in each cluster are set randomly to +1 or -1"
             const uint32_t dn = (pw[0] & 1u) | ((pw[1] & 1u) << 1) | ((pw[2] & 1u) << 2) | ((pw[3] & 1u) << 3);

@@ -46,7 +46,7 @@ struct RowGeom {
     static_assert(DIM == 2 || TY == 32, "3D: the 32 lanes of a warp are the 32 rows of one z-plane of the tile");
     static constexpr int NROWS = TY * TZ, NS = 32 * NROWS;
     static constexpr int LOG2NS = ilog2(NS);
-    static_assert((1 << LOG2NS) == NS && NS <= 32768, "tile sizes are powers of two; a node (2 x local index) fits 16 bits");
+    static_assert((1 << LOG2NS) == NS && NS <= 16384, "tile sizes are powers of two; the shared-window address of a parent entry fits 16 bits");
     static constexpr int NDIR = DIM - 1;                         // pending directions: y (and z)
     // face words: +x face one bit per row; +y face one word per z (the row y = TY-1); +z face one word per y
     static constexpr int FXW = NROWS / 32, FYW = TZ, FZW = (DIM == 3) ? TY : 0;
@@ -105,9 +105,9 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t saddr)
 }
 __device__ __forceinline__ uint32_t lds_u16(uint32_t saddr)
 {
-    uint16_t v;
-    asm volatile("ld.volatile.shared.u16 %0, [%1];" : "=h"(v) : "r"(saddr) : "memory");
-    return (uint32_t)v;
+    uint32_t v;   // (a 32-bit destination: the load zero-extends, no conversion instruction follows)
+    asm volatile("ld.volatile.shared.u16 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
+    return v;
 }
 // v <- 16-bit shared[saddr] if flag != 0 (predicated: no branch, no shared-memory wavefront when off)
 __device__ __forceinline__ void lds_u16_if(uint32_t &v, uint32_t flag, uint32_t saddr)
@@ -117,7 +117,7 @@ __device__ __forceinline__ void lds_u16_if(uint32_t &v, uint32_t flag, uint32_t 
 }
 __device__ __forceinline__ void sts_u16(uint32_t saddr, uint32_t v)
 {
-    asm volatile("st.volatile.shared.u16 [%0], %1;" :: "r"(saddr), "h"((uint16_t)v) : "memory");
+    asm volatile("st.volatile.shared.u16 [%0], %1;" :: "r"(saddr), "r"(v) : "memory");   // (the low 16 bits of v)
 }
 __device__ __forceinline__ uint32_t cas_shared(uint32_t saddr, uint32_t cmp, uint32_t val)
 {
@@ -157,7 +157,9 @@ __device__ __forceinline__ void union_nodes(uint32_t lab, uint32_t a, uint32_t b
 // start of the x-run of site x (below = mask of the bits under x): one past the highest inactive x-bond under it
 __device__ __forceinline__ uint32_t run_start(uint32_t bx, uint32_t below)
 {
-    return 32u - (uint32_t)__clz((int)(~bx & below));
+    uint32_t f;   // bfind: position of the highest set bit, 0xffffffff if there is none (one instruction; 32 - clz takes three)
+    asm("bfind.u32 %0, %1;" : "=r"(f) : "r"(~bx & below));
+    return f + 1u;
 }
 
 // The random decisions "u < P32" of the 32 x DIM bonds of group G (reading 6): X[k] bit b = decision
@@ -243,7 +245,11 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
     uint32_t *face_s = smem_u32 + G::OFF_FACE;
     uint32_t *fpre_s = smem_u32 + G::OFF_FPRE;        // NFW prefix counts, [NFWP] = base in the global pair list, [NFWP+1] = list length
     uint32_t *list_s = smem_u32 + G::OFF_LIST;
+    // A node of the tile-local forest is the shared-window ADDRESS of its 16-bit parent entry (lab_sa + 2 x local index;
+    // the entries are the first thing in dynamic shared memory, so the address fits 16 bits): an entry is followed with a
+    // load from the value just read, no base address is added in the loops.
     const uint32_t lab_sa = (uint32_t)__cvta_generic_to_shared(lab_s);
+    if (lab_sa + 2u * (uint32_t)G::NS > 65536u) __trap();
 
     const uint32_t L = p.L, LL = L * L;
     const uint32_t bx = blockIdx.x, by = blockIdx.y, bz = (DIM == 3) ? blockIdx.z : 0u;
@@ -427,7 +433,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
         // every site starts as its own root: its 16-bit parent entry = own node = 2 x local index.  Lanes
         // take the 16-byte pieces of their rows (64 bytes apart) in rotated order so that they spread
         // over all banks
-        const uint32_t o = (uint32_t)row * 64u;
+        const uint32_t o = lab_sa + (uint32_t)row * 64u;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const uint32_t jj = (uint32_t)(j + (lane >> 1)) & 3u;
@@ -476,7 +482,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
         // the two sites: nothing to do for it
         k.restY = sy & ~(k.first & ~k.sz) & ~((sy << 1) & (k.T << 1) & (k.bxY << 1));
         k.restZ = k.sz & ~k.first & ~((k.sz << 1) & (k.T << 1) & (k.bxZ << 1));
-        k.rowB = (uint32_t)row * 64u;
+        k.rowB = lab_sa + (uint32_t)row * 64u;
         return k;
     };
     uint32_t unfit = 0u;   // rows of this thread whose further bonds did not fit into the list
@@ -491,7 +497,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
             const bool isz = (DIM == 3) && (k.sz & low);   // a site reached from both rows takes the z bond
             const uint32_t b = k.rowB + 2u * run_start(k.T, below);
             const uint32_t a = (isz ? rowZ : rowY) + 2u * run_start(isz ? k.bxZ : k.bxY, below);
-            sts_u16(lab_sa + b, a);
+            sts_u16(b, a);
         }
         // the other bonds: (a, b) pairs for phase 2b, warp-aggregated reservation in the list
         const uint32_t cnt = __popc(k.restY) + __popc(k.restZ);
@@ -519,7 +525,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                         const uint32_t a = rowP + 2u * run_start(bxP, below);
                         // b has just been given a parent by this thread (a run with a further bond has a first
                         // one): the union starts from that parent, one level up
-                        list_s[pos++] = (a << 16) | lds_u16(lab_sa + b);
+                        list_s[pos++] = (a << 16) | lds_u16(b);
                     }
                 }
             } else {
@@ -558,18 +564,18 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 continue;   // every bond just fetched joins a run with its own parent: fetch again
             }
             if (a != b) {
-                const uint32_t pa = lds_u16(lab_sa + a), pb = lds_u16(lab_sa + b);
+                const uint32_t pa = lds_u16(a), pb = lds_u16(b);
                 if (pa == a && pb == b) {
                     const uint32_t hi = max(a, b), lo = min(a, b);
-                    const uint32_t old = cas_u16(lab_sa + hi, hi, lo);
+                    const uint32_t old = cas_u16(hi, hi, lo);
                     if (old == hi) a = b;                 // done
                     else { a = old; b = lo; }             // hi was hooked meanwhile: go on from its new parent
                 } else {
                     // climb two levels and make both nodes skip their parents (path halving: a non-root is
                     // never the target of a hook, and any ancestor is a valid parent)
-                    const uint32_t ga = lds_u16(lab_sa + pa), gb = lds_u16(lab_sa + pb);
-                    if (ga != pa) sts_u16(lab_sa + a, ga);
-                    if (gb != pb) sts_u16(lab_sa + b, gb);
+                    const uint32_t ga = lds_u16(pa), gb = lds_u16(pb);
+                    if (ga != pa) sts_u16(a, ga);
+                    if (gb != pb) sts_u16(b, gb);
                     a = ga; b = gb;                       // (a == b afterwards: same tree already)
                 }
             }
@@ -589,7 +595,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 while (w) {
                     const uint32_t low = w & (0u - w), below = low - 1u;
                     w ^= low;
-                    union_nodes(lab_sa, rowP + 2u * run_start(bxP, below), k.rowB + 2u * run_start(k.T, below));
+                    union_nodes(0u, rowP + 2u * run_start(bxP, below), k.rowB + 2u * run_start(k.T, below));
                 }
             }
         }
@@ -624,8 +630,8 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 const uint32_t ri = li_i >> 5;
                 uint32_t v = lds_u16(lab_sa + ri * 64u + 2u * run_start(bx_s[ri], (1u << (li_i & 31u)) - 1u));
 #pragma unroll
-                for (int k = 0; k < SW_ROW_JUMPS; ++k) v = lds_u16(lab_sa + v);
-                p.pairs[pos] = make_uint2(tile_base + (v >> 1), (tj << G::LOG2NS) + li_j);
+                for (int k = 0; k < SW_ROW_JUMPS; ++k) v = lds_u16(v);
+                p.pairs[pos] = make_uint2(tile_base + ((v - lab_sa) >> 1), (tj << G::LOG2NS) + li_j);
             }
         }
     }
@@ -644,14 +650,14 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 // first ancestor; if it is the run start itself the run start is a root and the site is done
                 // (no further loads: fewer shared-memory wavefronts; 45 % of the run starts are roots)
                 const uint32_t v0 = v;
-                v = lds_u16(lab_sa + v);
+                v = lds_u16(v);
                 const uint32_t more = (v != v0) ? 1u : 0u;
 #pragma unroll
-                for (int k = 1; k < SW_ROW_JUMPS; ++k) lds_u16_if(v, more, lab_sa + v);
+                for (int k = 1; k < SW_ROW_JUMPS; ++k) lds_u16_if(v, more, v);
             }
             uint32_t word;
-            if (MODEL != POTTS) word = (tile_base << 1) + v + ((dr_s[row] >> lane) & 1u);   // v = 2 x local index
-            else word = ((tile_base + (v >> 1)) << db) | reinterpret_cast<const uint8_t *>(dr_s)[row * 32 + lane];
+            if (MODEL != POTTS) word = ((tile_base << 1) - lab_sa) + v + ((dr_s[row] >> lane) & 1u);   // v - lab_sa = 2 x local index
+            else word = ((tile_base + ((v - lab_sa) >> 1)) << db) | reinterpret_cast<const uint8_t *>(dr_s)[row * 32 + lane];
             p.labels[tile_base + (uint32_t)row * 32u + (uint32_t)lane] = word;
         }
     }
