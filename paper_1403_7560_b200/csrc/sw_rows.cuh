@@ -36,6 +36,9 @@ namespace swk {
 // reading 6, domain GROUP: W_G[n] = word n % 4 of the call with counter word 3 = DOM_GROUP + 256 (n / 4)
 constexpr uint32_t GROUP_DRAW_BASE = 128u;
 
+#ifndef SW_ROW_UF_MERGED
+#define SW_ROW_UF_MERGED 1   // phase 2b: a climb that ends at two roots hooks them in the same round
+#endif
 #ifndef SW_ROW_JUMPS
 #define SW_ROW_JUMPS 3   // parent loads per site in phase 3 after the one of its run start
 #endif
@@ -564,6 +567,26 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 continue;   // every bond just fetched joins a run with its own parent: fetch again
             }
             if (a != b) {
+#if SW_ROW_UF_MERGED
+                // climb (two levels, path halving: a non-root is never the target of a hook, and any ancestor is
+                // a valid parent); if the parents turn out to be roots the hook follows in the same round
+                const uint32_t pa = lds_u16(a), pb = lds_u16(b);
+                bool roots = pa == a && pb == b;
+                if (!roots) {
+                    const uint32_t ga = lds_u16(pa), gb = lds_u16(pb);
+                    if (ga != pa) sts_u16(a, ga);
+                    if (gb != pb) sts_u16(b, gb);
+                    roots = ga == pa && gb == pb;
+                    a = roots ? pa : ga;
+                    b = roots ? pb : gb;                  // (a == b afterwards: same tree already)
+                }
+                if (roots && a != b) {
+                    const uint32_t hi = max(a, b), lo = min(a, b);
+                    const uint32_t old = cas_u16(hi, hi, lo);
+                    if (old == hi) a = b;                 // done
+                    else { a = old; b = lo; }             // hi was hooked meanwhile: go on from its new parent
+                }
+#else
                 const uint32_t pa = lds_u16(a), pb = lds_u16(b);
                 if (pa == a && pb == b) {
                     const uint32_t hi = max(a, b), lo = min(a, b);
@@ -578,6 +601,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                     if (gb != pb) sts_u16(b, gb);
                     a = ga; b = gb;                       // (a == b afterwards: same tree already)
                 }
+#endif
             }
         }
     

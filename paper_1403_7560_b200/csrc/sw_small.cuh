@@ -283,17 +283,22 @@ __global__ void __launch_bounds__(1024, 1) k_sw_small(const Params p, const Smal
                         continue;
                     }
                     if (a != b) {
+                        // climb two levels (path halving); if the parents turn out to be roots, hook in the same round
                         const uint32_t pa = lds_u16(lab_sa + a), pb = lds_u16(lab_sa + b);
-                        if (pa == a && pb == b) {
+                        bool roots = pa == a && pb == b;
+                        if (!roots) {
+                            const uint32_t ga = lds_u16(lab_sa + pa), gb = lds_u16(lab_sa + pb);
+                            if (ga != pa) sts_u16(lab_sa + a, ga);
+                            if (gb != pb) sts_u16(lab_sa + b, gb);
+                            roots = ga == pa && gb == pb;
+                            a = roots ? pa : ga;
+                            b = roots ? pb : gb;
+                        }
+                        if (roots && a != b) {
                             const uint32_t hi = max(a, b), lo = min(a, b);
                             const uint32_t old = cas_u16(lab_sa + hi, hi, lo);
                             if (old == hi) a = b;
                             else { a = old; b = lo; }
-                        } else {
-                            const uint32_t ga = lds_u16(lab_sa + pa), gb = lds_u16(lab_sa + pb);
-                            if (ga != pa) sts_u16(lab_sa + a, ga);
-                            if (gb != pb) sts_u16(lab_sa + b, gb);
-                            a = ga; b = gb;
                         }
                     }
                 }
