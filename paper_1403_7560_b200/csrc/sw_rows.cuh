@@ -13,7 +13,8 @@
 //             spins), three ballots per row give the same masks.
 //             Bx gives the x-runs of the row with no union at all.  Bonds through the tile faces go to face
 //             words (-> global pair list, k_merge).  Nodes of the tile-local union-find are the RUN STARTS;
-//             the run start of a site is a find-leading-one on the row's Bx mask.  16-bit parent entries.
+//             the run start of a site is one bfind on the row's Bx mask.  16-bit parent entries that hold the
+//             shared-window address of the parent's entry (a chain is followed with no address arithmetic).
 //   phase 2a  [thread = row] "pull": every run looks back at the bonds that reach it from the row below
 //             (y - 1) and the row behind (z - 1); the first such bond of the run makes the run start it
 //             comes from the parent of this run start -- a plain store, no atomic, no retry, because only
@@ -142,7 +143,8 @@ __device__ __forceinline__ uint32_t cas_u16(uint32_t saddr, uint32_t cmp, uint32
         old = got;
     }
 }
-// Lock-free union of the trees of nodes a and b.  A node is 2 x the tile-local index of a run start; its
+// Lock-free union of the trees of nodes a and b.  A node is 2 x the local index of a run start (k_sw_small; lab = the
+// shared-window address of the entries) or the shared-window address of its entry itself (k_bond_label_rows; lab = 0); its
 // 16-bit parent entry sits at lab + node; a root points to itself; every link hangs the larger root under
 // a smaller node, so the root of a tree is its minimum index.
 __device__ __forceinline__ void union_nodes(uint32_t lab, uint32_t a, uint32_t b)
@@ -433,7 +435,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 dr_s[row * 8 + j] = d;
             }
         }
-        // every site starts as its own root: its 16-bit parent entry = own node = 2 x local index.  Lanes
+        // every site starts as its own root: its 16-bit parent entry = own node = the address of that entry.  Lanes
         // take the 16-byte pieces of their rows (64 bytes apart) in rotated order so that they spread
         // over all banks
         const uint32_t o = lab_sa + (uint32_t)row * 64u;
