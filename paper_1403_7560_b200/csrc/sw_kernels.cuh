@@ -37,7 +37,15 @@
 #endif
 #if SW_XY_FAST_MATH
 #define SW_SINCOSF(x, s, c) __sincosf((x), (s), (c))
-#define SW_NEG_EXPM1F(x) (1.0f - __expf(x))
+// 1 - exp(x) for x <= 0 (x = -2 beta a_i a_j): __expf is ex2.approx(x log2 e) plus a rescaling for results below 2^-126, which
+// 1 - r rounds to 1.0f either way; the .ftz form of the same SFU instruction gives the same bits without the rescaling.
+__device__ __forceinline__ float sw_exp_le0(float x)
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x * 1.4426950408889634f));
+    return r;
+}
+#define SW_NEG_EXPM1F(x) (1.0f - sw_exp_le0(x))
 #else
 #define SW_SINCOSF(x, s, c) sincosf((x), (s), (c))
 #define SW_NEG_EXPM1F(x) (-expm1f(x))

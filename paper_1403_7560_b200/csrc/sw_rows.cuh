@@ -345,6 +345,9 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 if (gy >= L) gup -= L * L;                                  // wrapped: back by L rows
             }
             float aprev = proj(gxl + gup);
+            // the +z neighbour of a site of this plane is a fixed distance away (periodic wrap: back by L - 1 planes)
+            uint32_t dzoff = (z0 + (uint32_t)lz + 1u == L) ? 0u - LL * (L - 1u) : LL;
+            asm volatile("" : "+r"(dzoff));   // (kept in a register: otherwise it is recomputed from blockIdx in every iteration)
 #pragma unroll 1
             for (int yy = 31; yy >= 0; --yy) {
                 const uint32_t grow_ = rowbase0 + L * (uint32_t)yy;
@@ -357,8 +360,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 const uint32_t my = __ballot_sync(FULL, decide(a, aprev, w.y));
                 uint32_t mz = 0u;
                 if (DIM == 3) {
-                    const uint32_t gzn = (z0 + (uint32_t)lz + 1u == L) ? site - LL * (L - 1u) : site + LL;
-                    mz = __ballot_sync(FULL, decide(a, proj(gzn), w.z));
+                    mz = __ballot_sync(FULL, decide(a, proj(site + dzoff), w.z));
                 }
                 const uint32_t md = __ballot_sync(FULL, (w.w >> 31) != 0u);
                 if (lane == yy) { Bx = mx; By = my; Bz = mz; D = md; }
