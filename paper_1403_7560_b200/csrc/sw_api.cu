@@ -524,6 +524,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     }
     p.L = (uint32_t)L; p.N = (uint32_t)c->N;
     p.k0 = (uint32_t)(seed & 0xffffffffu); p.k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) { p.rk[2 * r] = p.k0 + (uint32_t)r * 0x9E3779B9u; p.rk[2 * r + 1] = p.k1 + (uint32_t)r * 0xBB67AE85u; }
     // PAPER.md:96 (garbled "p = 1 e^{2J/T}"): Ising p = 1 - exp(-2 beta); PAPER.md:152 + Eq. 2: Potts
     // p = 1 - exp(-beta).  The decision is the integer compare word < floor(p 2^32).
     const double prob = (model == SW_ISING) ? -std::expm1(-2.0 * beta) : -std::expm1(-beta);

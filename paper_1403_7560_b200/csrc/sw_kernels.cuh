@@ -98,6 +98,7 @@ struct Params {
     uint32_t L, N;
     uint32_t ntx, nty, ntz, ntiles;
     uint32_t k0, k1;   // Philox key = (seed low, seed high)
+    uint32_t rk[20];   // its ten round keys (k0 + r 0x9E3779B9, k1 + r 0xBB67AE85), r = 0..9: constant-bank operands for the per-site generator
     uint32_t P32;      // Ising/Potts: bond active iff word < P32
     int q;
     int db;            // draw bits in a label word: 1 (Ising, XY), ceil(log2 q) (Potts)
@@ -124,6 +125,24 @@ __host__ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1
         c2 = n2;
         k0 += 0x9E3779B9u;
         k1 += 0xBB67AE85u;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// The same numbers with the round keys read from the kernel parameters (constant bank): a loop that makes one call per
+// iteration (XY, clock: one call per site) otherwise redoes the 18 key additions in every iteration.
+__device__ __forceinline__ uint4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const Params &p)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned long long a = 0xD2511F53ull * c0;
+        const unsigned long long b = 0xCD9E8D57ull * c2;
+        const uint32_t n0 = (uint32_t)(b >> 32) ^ c1 ^ p.rk[2 * r];
+        const uint32_t n2 = (uint32_t)(a >> 32) ^ c3 ^ p.rk[2 * r + 1];
+        c1 = (uint32_t)b;
+        c3 = (uint32_t)a;
+        c0 = n0;
+        c2 = n2;
     }
     return make_uint4(c0, c1, c2, c3);
 }

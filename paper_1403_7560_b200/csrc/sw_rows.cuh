@@ -330,8 +330,11 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
             };
             auto decide = [&](float a, float b, uint32_t word) -> bool {
                 if (MODEL == XY) {
+                    // (no short-circuit: for pr <= 0 the right-hand side is <= 0 and the comparison false anyway; a warp
+                    // has a site with pr > 0 in practically every row, so the branch saved nothing)
                     const float pr = a * b;
-                    return pr > 0.f && (float)(word >> 8) * 5.9604644775390625e-8f < SW_NEG_EXPM1F(p.m2beta * pr);
+                    const bool below = (float)(word >> 8) * 5.9604644775390625e-8f < SW_NEG_EXPM1F(p.m2beta * pr);
+                    return (pr > 0.f) & below;
                 } else {
                     const uint32_t ca = __float_as_uint(a), cb = __float_as_uint(b);
                     if (((ca & cb) >> 16) == 0u) return false;        // different sign, or one component is zero
@@ -355,7 +358,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 const float a = proj(site);
                 float ax = __shfl_down_sync(FULL, a, 1);
                 if (lane == 31) ax = proj(xh + grow_);
-                const uint4 w = philox4x32_10(site, t_lo, t_hi, DOM_SITE, p.k0, p.k1);
+                const uint4 w = philox4x32_10_rk(site, t_lo, t_hi, DOM_SITE, p);
                 const uint32_t mx = __ballot_sync(FULL, decide(a, ax, w.x));
                 const uint32_t my = __ballot_sync(FULL, decide(a, aprev, w.y));
                 uint32_t mz = 0u;
