@@ -759,6 +759,9 @@ __device__ __forceinline__ uint4 ldg_stream(const uint32_t *ptr)
 // L1; further hops only for clusters that cross tile faces), takes the root's draw field as the
 // cluster's new value and writes its spin; magnetisation sums per CTA.
 // ------------------------------------------------------------------------------------------------
+#ifndef SW_FLIP_FIRST_HOP_ALWAYS
+#define SW_FLIP_FIRST_HOP_ALWAYS 1
+#endif
 #ifndef SW_FLIP_PREFETCH
 #define SW_FLIP_PREFETCH 1   // quads whose label words are in flight ahead of the chase
 #endif
@@ -833,7 +836,11 @@ __global__ void __launch_bounds__(NT, (SW_FLIP_THREADS_PER_SM / NT > 0 ? SW_FLIP
 #pragma unroll
         for (int s = 0; s < 4; ++s) {
             at[s] = pw[s] >> db;
+#if SW_FLIP_FIRST_HOP_ALWAYS
+            pw[s] = __ldg(lab + at[s]);     // (a site that is its own ancestor reads its own word again: an L1 hit, no predicate)
+#else
             if (at[s] != a0 + (uint32_t)s) pw[s] = __ldg(lab + at[s]);
+#endif
         }
         for (;;) {
             const uint32_t q0 = pw[0] >> db, q1 = pw[1] >> db, q2 = pw[2] >> db, q3 = pw[3] >> db;
