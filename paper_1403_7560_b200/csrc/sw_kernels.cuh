@@ -807,6 +807,7 @@ __global__ void __launch_bounds__(NT, (SW_FLIP_THREADS_PER_SM / NT > 0 ? SW_FLIP
         g_first = (x0 + lx) + L * ((y0 + ly) + L * (z0 + lz));
         g_step = STEP_PLANES > 0 ? (uint32_t)STEP_PLANES * L * L : (uint32_t)STEP_ROWS * L;
     }
+    asm volatile("" : "+r"(g_first));   // (kept in a register: otherwise it is rebuilt from threadIdx / blockIdx for every quad)
     // the label words of the NEXT quad are requested before the parents of this one are followed: the
     // kernel is bound by the latency of these reads (DRAM), not by instruction issue
 #if SW_FLIP_PREFETCH == 2
