@@ -66,11 +66,11 @@ def kernel_bytes_per_site(model):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the `ncu --set full` captures summarised
 # under profiles/ (config -> kernel -> bytes); lts__t_bytes for the L2-sized configs is in the same files.
 NCU_TRAFFIC = {
-    "C4": {"k_bond_label": 134.5e6 + 510.4e6, "k_merge": 348.9e6 + 69.4e6, "k_flip": 537.9e6 + 119.7e6},
-    "C2": {"k_bond_label": 16.8e6 + 13.6e6, "k_merge": 49.0e6 + 0.2e6, "k_flip": 67.1e6 + 3.3e6},
-    "C5": {"k_bond_label": 67.4e6 + 23.7e6, "k_merge": 38.5e6 + 0.1e6, "k_flip": 134.5e6 + 21.0e6},
-    "X3": {"k_bond_label": 34.2e6 + 15.5e6, "k_merge": 38.6e6 + 0.1e6, "k_flip": 100.8e6 + 5.9e6},
-    "C1": {"k_sw_small": 35.6e3 / 200},
+    "C4": {"k_bond_label": 134.6e6 + 511.9e6, "k_merge": 348.9e6 + 69.4e6, "k_flip": 537.9e6 + 119.7e6},
+    "C2": {"k_bond_label": 16.8e6 + 12.1e6, "k_merge": 49.0e6 + 0.3e6, "k_flip": 67.1e6 + 3.7e6},
+    "C5": {"k_bond_label": 67.4e6 + 23.9e6, "k_merge": 38.6e6 + 0.1e6, "k_flip": 134.5e6 + 20.3e6},
+    "X3": {"k_bond_label": 34.2e6 + 14.7e6, "k_merge": 38.7e6 + 0.1e6, "k_flip": 100.8e6 + 6.3e6},
+    "C1": {"k_sw_small": 35.8e3 / 200},
 }
 NCU_TRAFFIC_SOURCE = {"C4": "profiles/r02_ncu_full_C4.md (ncu --set full, per launch)",
                       "C2": "profiles/r02_ncu_full_C2_C5_X3_C1.md (cold L2; L2 bytes in the same file)",
