@@ -343,7 +343,9 @@ void launch_measure_dm(sw_ctx *c, bool with_m)
         if (with_m) k_measure_xy<DIM, true><<<g, 256, 0, c->stream>>>(c->p);
         else k_measure_xy<DIM, false><<<g, 256, 0, c->stream>>>(c->p);
     } else {
-        const unsigned g = (unsigned)(c->N / 1024);  // four sites per thread
+        unsigned g = (unsigned)(c->N / 4096);        // 16 sites per thread and iteration, grid-stride
+        if (g < 1u) g = 1u;
+        if (g > 148u * 8u) g = 148u * 8u;            // a CTA adds to the global sums once
         if (with_m) k_measure4<DIM, MODEL, true><<<g, 256, 0, c->stream>>>(c->p);
         else k_measure4<DIM, MODEL, false><<<g, 256, 0, c->stream>>>(c->p);
     }

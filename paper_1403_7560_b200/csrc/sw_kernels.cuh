@@ -1018,58 +1018,77 @@ __global__ void __launch_bounds__(256) k_measure_xy(const Params p)
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_measure4 (Ising, Potts): E (Eq. 1, 2) and, if WITH_M, the magnetisation sums (Eq. 4, 5); four consecutive sites per thread.  The spin words of the
-// quad and of its +x / +y / +z neighbours give byte-equality masks; with spins in the model's range
-// the energy is a popcount: Ising -sum s_i s_j = (#pairs - 2 #equal), Potts #unequal pairs.
+// k_measure4 (Ising, Potts): E (Eq. 1, 2) and, if WITH_M, the magnetisation sums (Eq. 4, 5).  Grid-stride over
+// groups of 16 consecutive sites (L is a multiple of 32), 16-byte loads; the spin words of the group and of its
+// +x / +y / +z neighbours give byte-equality masks, and with spins in the model's range the energy is a popcount:
+// Ising -sum s_i s_j = (#pairs - 2 #equal), Potts #unequal pairs.  A CTA adds to the global sums once, at its
+// end (one atomic per 1024 sites on a single address was what bounded the first version of this kernel).
 // ------------------------------------------------------------------------------------------------
 template <int DIM, int MODEL, bool WITH_M>
 __global__ void __launch_bounds__(256) k_measure4(const Params p)
 {
     __shared__ uint32_t hist_s[256];
-    __shared__ int red_s[2][8];
+    __shared__ long long red_s[2][8];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t L = p.L, LL = L * L;
-    const uint32_t g = (blockIdx.x * 256u + tid) * 4u;  // N is a multiple of 1024
     if (MODEL == POTTS && WITH_M) {
         hist_s[tid] = 0u;
         __syncthreads();
     }
-    uint32_t x, y, z;
-    decode(p, g, x, y, z);
     const uint8_t *sp = (const uint8_t *)p.spins;
-    const uint32_t own = *reinterpret_cast<const uint32_t *>(sp + g);
-    const uint32_t nb = sp[(x + 4 == L) ? g + 4 - L : g + 4];
-    const uint32_t up = *reinterpret_cast<const uint32_t *>(sp + ((y + 1 == L) ? g - L * (L - 1) : g + L));
-    int equal = __popc(eq4(own, __funnelshift_r(own, nb, 8))) + __popc(eq4(own, up));
-    if (DIM == 3) {
-        const uint32_t fr = *reinterpret_cast<const uint32_t *>(sp + ((z + 1 == L) ? g - LL * (L - 1) : g + LL));
-        equal += __popc(eq4(own, fr));
-    }
-    int e = (MODEL == ISING) ? 4 * DIM - 2 * equal : 4 * DIM - equal;
-    int m = 0;
-    if (WITH_M) {
-        if (MODEL == ISING) {
-            m = 4 - 2 * __popc(own & 0x80808080u);  // +1 = 0x01, -1 = 0xff
-        } else if (p.q <= 8) {
-            uint32_t lo = 0u, hi = 0u;
+    const uint32_t ngroups = p.N >> 4;
+    long long e_acc = 0, m_acc = 0;
+    for (uint32_t q = blockIdx.x * 256u + (uint32_t)tid; q < ngroups; q += gridDim.x * 256u) {
+        const uint32_t g = q << 4;
+        uint32_t x, y, z;
+        decode(p, g, x, y, z);
+        const uint4 own = *reinterpret_cast<const uint4 *>(sp + g);
+        const uint32_t nb = sp[(x + 16 == L) ? g + 16 - L : g + 16];
+        const uint4 up = *reinterpret_cast<const uint4 *>(sp + ((y + 1 == L) ? g - L * (L - 1) : g + L));
+        int equal = __popc(eq4(own.x, __funnelshift_r(own.x, own.y, 8))) + __popc(eq4(own.y, __funnelshift_r(own.y, own.z, 8))) +
+                    __popc(eq4(own.z, __funnelshift_r(own.z, own.w, 8))) + __popc(eq4(own.w, __funnelshift_r(own.w, nb, 8))) +
+                    __popc(eq4(own.x, up.x)) + __popc(eq4(own.y, up.y)) + __popc(eq4(own.z, up.z)) + __popc(eq4(own.w, up.w));
+        if (DIM == 3) {
+            const uint4 fr = *reinterpret_cast<const uint4 *>(sp + ((z + 1 == L) ? g - LL * (L - 1) : g + LL));
+            equal += __popc(eq4(own.x, fr.x)) + __popc(eq4(own.y, fr.y)) + __popc(eq4(own.z, fr.z)) + __popc(eq4(own.w, fr.w));
+        }
+        e_acc += (MODEL == ISING) ? 16 * DIM - 2 * equal : 16 * DIM - equal;
+        if (WITH_M) {
+            const uint32_t ow[4] = {own.x, own.y, own.z, own.w};
+            if (MODEL == ISING) {
+                m_acc += 16 - 2 * (__popc(own.x & 0x80808080u) + __popc(own.y & 0x80808080u) + __popc(own.z & 0x80808080u) +
+                                   __popc(own.w & 0x80808080u));  // +1 = 0x01, -1 = 0xff
+            } else if (p.q <= 8) {
+                // (every thread of the warp is in the loop or none: ngroups is a multiple of 64)
+                uint32_t lo = 0u, hi = 0u;   // per-thread counts of states 0-3 / 4-7, one byte each (16 sites: no overflow)
 #pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                const uint32_t v = (own >> (8 * s)) & 0xffu, inc = 1u << ((v & 3u) * 8u);
-                if (v & 4u) hi += inc; else lo += inc;
-            }
-            for (int k = 0; k < p.q; ++k) {
-                const uint32_t c = ((k < 4 ? lo : hi) >> ((k & 3) * 8)) & 0xffu;
-                const uint32_t w = __reduce_add_sync(FULL, c);
-                if (lane == 0 && w) atomicAdd(&hist_s[k], w);
-            }
-        } else {
+                for (int w = 0; w < 4; ++w) {
 #pragma unroll
-            for (int s = 0; s < 4; ++s) atomicAdd(&hist_s[(own >> (8 * s)) & 0xffu], 1u);
+                    for (int b = 0; b < 4; ++b) {
+                        const uint32_t v = (ow[w] >> (8 * b)) & 0xffu, inc = 1u << ((v & 3u) * 8u);
+                        if (v & 4u) hi += inc; else lo += inc;
+                    }
+                }
+                for (int k = 0; k < p.q; ++k) {
+                    const uint32_t c = ((k < 4 ? lo : hi) >> ((k & 3) * 8)) & 0xffu;
+                    const uint32_t w = __reduce_add_sync(FULL, c);
+                    if (lane == 0 && w) atomicAdd(&hist_s[k], w);
+                }
+            } else {
+#pragma unroll
+                for (int w = 0; w < 4; ++w) {
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) atomicAdd(&hist_s[(ow[w] >> (8 * b)) & 0xffu], 1u);
+                }
+            }
         }
     }
-    e = __reduce_add_sync(FULL, e);
-    m = __reduce_add_sync(FULL, m);
-    if (lane == 0) { red_s[0][warp] = e; red_s[1][warp] = m; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        e_acc += __shfl_down_sync(FULL, e_acc, o);
+        m_acc += __shfl_down_sync(FULL, m_acc, o);
+    }
+    if (lane == 0) { red_s[0][warp] = e_acc; red_s[1][warp] = m_acc; }
     __syncthreads();
     if (tid == 0) {
         long long es = 0, ms = 0;
