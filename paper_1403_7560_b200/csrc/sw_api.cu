@@ -508,7 +508,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
     p.ntiles = p.ntx * p.nty * p.ntz;
     p.db = draw_bits(model, q);
     {   // k_merge: grid-stride loop over the pair list.  The grid is fixed at create time (graph replay) from
-        // the capacity of the list; 64 CTAs per SM leave one or two pairs per thread at T_c, so that CTAs
+        // the capacity of the list; 96 CTAs per SM leave about one pair per thread at T_c, so that CTAs
         // run through the list in order (the list is in tile order: neighbouring pairs touch neighbouring
         // label blocks, which stay in L2).  A resident grid (8 CTAs per SM, 13 pairs per thread) sweeps the
         // whole label array 13 times instead: C4 k_merge 0.264 ms vs 0.138 ms.
@@ -517,7 +517,7 @@ int create_common(sw_ctx **out, int dim, int L, int model, int q, double beta, u
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         const size_t max_pairs = c->N / c->ops.tx + c->N / c->ops.ty + (dim == 3 ? c->N / c->ops.tz : 0);
         size_t blocks = (max_pairs + 255) / 256;
-        if (blocks > (size_t)sms * 64) blocks = (size_t)sms * 64;
+        if (blocks > (size_t)sms * 96) blocks = (size_t)sms * 96;   // (C4: 64 / 80 / 96 / 112 CTAs per SM: 0.133 / 0.133 / 0.129 / 0.136 ms)
         if (const char *env = std::getenv("SW_B200_MERGE_BLOCKS")) {   // test knob: another interleaving of the unions
             const long v = std::atol(env);
             if (v >= 1 && v <= 65535 * 16) blocks = (size_t)v;

@@ -683,7 +683,7 @@ __device__ __forceinline__ uint32_t linear_of(const Params &p, uint32_t a)
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_merge: grid-stride loop over the compact pair list (grid: 64 CTAs per SM, i.e. one or two pairs per
+// k_merge: grid-stride loop over the compact pair list (grid: 96 CTAs per SM, i.e. one or two pairs per
 // thread, so that the list - which is in tile order - is walked in order and label blocks stay in L2).  Union of (a, b): both chains are followed in
 // one loop (two loads in flight), path splitting on the way (non-roots are re-pointed to their
 // grandparent with relaxed atomic stores, keeping their draw field); then the root with the larger linear
