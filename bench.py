@@ -66,8 +66,8 @@ def kernel_bytes_per_site(model):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the `ncu --set full` captures summarised
 # under profiles/ (config -> kernel -> bytes); lts__t_bytes for the L2-sized configs is in the same files.
 NCU_TRAFFIC = {
-    "C4": {"k_bond_label": 134.6e6 + 511.9e6, "k_merge": 348.9e6 + 69.4e6, "k_flip": 537.9e6 + 119.7e6},
-    "C2": {"k_bond_label": 16.8e6 + 12.1e6, "k_merge": 49.0e6 + 0.3e6, "k_flip": 67.1e6 + 3.7e6},
+    "C4": {"k_bond_label": 134.5e6 + 509.3e6, "k_merge": 348.1e6 + 68.4e6, "k_flip": 538.0e6 + 119.9e6},
+    "C2": {"k_bond_label": 16.8e6 + 12.9e6, "k_merge": 49.0e6 + 0.2e6, "k_flip": 67.1e6 + 3.2e6},
     "C5": {"k_bond_label": 67.4e6 + 23.9e6, "k_merge": 38.6e6 + 0.1e6, "k_flip": 134.5e6 + 20.3e6},
     "X3": {"k_bond_label": 34.2e6 + 14.7e6, "k_merge": 38.7e6 + 0.1e6, "k_flip": 100.8e6 + 6.3e6},
     "C1": {"k_sw_small": 35.8e3 / 200},
