@@ -43,6 +43,9 @@ constexpr uint32_t GROUP_DRAW_BASE = 128u;
 #ifndef SW_ROW_EARLY_RANDOM
 #define SW_ROW_EARLY_RANDOM 1   // 2D Ising / Potts, R = 1: the row's random decisions before the spins arrive
 #endif
+#ifndef SW_ROW_P3_UNROLL
+#define SW_ROW_P3_UNROLL 4   // rows of phase 3 in flight per warp (1 / 2 / 4: C2 kernel 0.0632 / 0.0614 / 0.0600 ms, C4 0.447 / 0.439 / 0.439)
+#endif
 #ifndef SW_ROW_JUMPS
 #define SW_ROW_JUMPS 3   // parent loads per site in phase 3 after the one of its run start
 #endif
@@ -697,7 +700,13 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
     {
         const int db = (MODEL == POTTS) ? p.db : 1;
         const uint32_t below = (1u << lane) - 1u;
+#if SW_ROW_P3_UNROLL == 4
+#pragma unroll 4
+#elif SW_ROW_P3_UNROLL == 1
+#pragma unroll 1
+#else
 #pragma unroll 2
+#endif
         for (int row = warp; row < NROWS; row += NW) {
             const uint32_t st = run_start(bx_s[row], below);
             uint32_t v = lds_u16(lab_sa + (uint32_t)row * 64u + 2u * st);
