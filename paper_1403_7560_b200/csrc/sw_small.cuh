@@ -130,14 +130,13 @@ __global__ void __launch_bounds__(1024, 1) k_sw_small(const Params p, const Smal
     // thread and step).  The pull leaves chains as long as a cluster is wide in y + z (at T_c: the lattice
     // size); each pass halves them before the root chase of the flip phase.
     auto jump_pass = [&]() {
-        for (uint32_t v = (uint32_t)tid; v < N / 8u; v += blockDim.x) {
-            const uint4 w = *reinterpret_cast<const uint4 *>(lab_s + 4u * v);
-            uint4 o;
+        // (four entries per thread: all 1024 threads work on a 4096-site lattice)
+        for (uint32_t v = (uint32_t)tid; v < N / 4u; v += blockDim.x) {
+            const uint2 w = *reinterpret_cast<const uint2 *>(lab_s + 2u * v);
+            uint2 o;
             o.x = lds_u16(lab_sa + (w.x & 0xffffu)) | (lds_u16(lab_sa + (w.x >> 16)) << 16);
             o.y = lds_u16(lab_sa + (w.y & 0xffffu)) | (lds_u16(lab_sa + (w.y >> 16)) << 16);
-            o.z = lds_u16(lab_sa + (w.z & 0xffffu)) | (lds_u16(lab_sa + (w.z >> 16)) << 16);
-            o.w = lds_u16(lab_sa + (w.w & 0xffffu)) | (lds_u16(lab_sa + (w.w >> 16)) << 16);
-            *reinterpret_cast<uint4 *>(lab_s + 4u * v) = o;
+            *reinterpret_cast<uint2 *>(lab_s + 2u * v) = o;
         }
         __syncthreads();
     };
@@ -328,29 +327,46 @@ __global__ void __launch_bounds__(1024, 1) k_sw_small(const Params p, const Smal
         {
             const uint32_t below = (1u << lane) - 1u;
             int m_loc = 0;
-            for (uint32_t row = (uint32_t)warp; row < NR; row += (uint32_t)NW) {
-                uint32_t v = lds_u16(lab_sa + row * 64u + 2u * run_start(bx_s[row], below));
-                for (;;) {
-                    const uint32_t n = lds_u16(lab_sa + v);
-                    if (n == v) break;
-                    v = n;
+            // four rows of a warp in flight: the chases are chains of dependent shared-memory loads
+#pragma unroll 1
+            for (uint32_t row0 = (uint32_t)warp; row0 < NR; row0 += 4u * (uint32_t)NW) {
+                uint32_t v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint32_t row = row0 + (uint32_t)j * (uint32_t)NW;
+                    v[j] = row < NR ? lds_u16(lab_sa + row * 64u + 2u * run_start(bx_s[row], below)) : 0u;   // (node 0 is a root)
                 }
-                const uint32_t root = v >> 1;                       // linear index of the root
-                if (MODEL == ISING) {
-                    const uint32_t d = (dr_s[root >> 5] >> (root & 31u)) & 1u;   // 1: the cluster becomes +1
-                    const uint32_t plus = __ballot_sync(FULL, d);
-                    if (lane == 0) st_s[row] = ~plus;                // sign masks: bit set = spin -1
-                    m_loc += 2 * __popc(plus) - 32;
-                    if (last && args.write_labels) {
-                        const uint32_t own = (dr_s[row] >> lane) & 1u;
-                        p.labels[row * 32u + (uint32_t)lane] = (root << 1) | own;
+                for (;;) {
+                    uint32_t nn[4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) nn[j] = lds_u16(lab_sa + v[j]);
+                    const bool done = nn[0] == v[0] && nn[1] == v[1] && nn[2] == v[2] && nn[3] == v[3];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) v[j] = nn[j];
+                    if (done) break;
+                }
+                __syncwarp();
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint32_t row = row0 + (uint32_t)j * (uint32_t)NW;
+                    if (row >= NR) break;                            // (uniform in the warp)
+                    const uint32_t root = v[j] >> 1;                 // linear index of the root
+                    if (MODEL == ISING) {
+                        const uint32_t d = (dr_s[root >> 5] >> (root & 31u)) & 1u;   // 1: the cluster becomes +1
+                        const uint32_t plus = __ballot_sync(FULL, d);
+                        if (lane == 0) st_s[row] = ~plus;                // sign masks: bit set = spin -1
+                        m_loc += 2 * __popc(plus) - 32;
+                        if (last && args.write_labels) {
+                            const uint32_t own = (dr_s[row] >> lane) & 1u;
+                            p.labels[row * 32u + (uint32_t)lane] = (root << 1) | own;
+                        }
+                    } else {
+                        const uint32_t d = reinterpret_cast<const uint8_t *>(dr_s)[root];
+                        reinterpret_cast<uint8_t *>(st_s)[row * 32u + (uint32_t)lane] = (uint8_t)d;
+                        atomicAdd(&misc_s[8 + d], 1u);
+                        if (last && args.write_labels)
+                            p.labels[row * 32u + (uint32_t)lane] = (root << db) | reinterpret_cast<const uint8_t *>(dr_s)[row * 32u + (uint32_t)lane];
                     }
-                } else {
-                    const uint32_t d = reinterpret_cast<const uint8_t *>(dr_s)[root];
-                    reinterpret_cast<uint8_t *>(st_s)[row * 32u + (uint32_t)lane] = (uint8_t)d;
-                    atomicAdd(&misc_s[8 + d], 1u);
-                    if (last && args.write_labels)
-                        p.labels[row * 32u + (uint32_t)lane] = (root << db) | reinterpret_cast<const uint8_t *>(dr_s)[row * 32u + (uint32_t)lane];
                 }
             }
             if (MODEL == ISING && lane == 0) atomicAdd(reinterpret_cast<unsigned long long *>(misc_s + 4), (unsigned long long)(long long)m_loc);
