@@ -165,6 +165,27 @@ __device__ __forceinline__ void union_nodes(uint32_t lab, uint32_t a, uint32_t b
         a = old; b = lo;
     }
 }
+// The same with path halving on the way up (every node visited is re-pointed to its grandparent: a non-root is never
+// the target of a hook, and any ancestor is a valid parent) -- for the bonds that found no room in the list (ordered
+// phase), which a thread works off one after the other.
+__device__ __forceinline__ void union_nodes_halving(uint32_t a, uint32_t b)
+{
+    for (;;) {
+        for (;;) {
+            const uint32_t pa = lds_u16(a), pb = lds_u16(b);
+            if (pa == a && pb == b) break;
+            const uint32_t ga = lds_u16(pa), gb = lds_u16(pb);
+            if (ga != pa) sts_u16(a, ga);
+            if (gb != pb) sts_u16(b, gb);
+            a = ga; b = gb;
+        }
+        if (a == b) return;
+        const uint32_t hi = max(a, b), lo = min(a, b);
+        const uint32_t old = cas_u16(hi, hi, lo);
+        if (old == hi) return;
+        a = old; b = lo;
+    }
+}
 // start of the x-run of site x (below = mask of the bits under x): one past the highest inactive x-bond under it
 __device__ __forceinline__ uint32_t run_start(uint32_t bx, uint32_t below)
 {
@@ -653,7 +674,7 @@ __global__ void __launch_bounds__((RowKernelTraits<DIM, MODEL, TY, TZ, R>::NT), 
                 while (w) {
                     const uint32_t low = w & (0u - w), below = low - 1u;
                     w ^= low;
-                    union_nodes(0u, rowP + 2u * run_start(bxP, below), k.rowB + 2u * run_start(k.T, below));
+                    union_nodes_halving(rowP + 2u * run_start(bxP, below), k.rowB + 2u * run_start(k.T, below));
                 }
             }
         }
